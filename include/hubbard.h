@@ -1,0 +1,190 @@
+/*
+ * hubbard.h — C ABI of libhubbard_b200: the hot path of Siro & Harju,
+ * "Exact diagonalization of the Hubbard model on graphics processing units"
+ * (arxiv 1204.3425) for NVIDIA B200 (sm_100a).
+ *
+ * What the library computes
+ *   H = -t sum_<ij>,s (c+_is c_js + h.c.) + U sum_i n_iup n_idn       PAPER.md:23 (eq. 1-2)
+ *   in the fixed (N_up, N_dn) sector, basis ordered as in
+ *   PAPER.md:41-71 (eq. 4-8): up operators left of down operators, sites
+ *   ascending, state index J = i_up * dim_dn + i_dn with i_s the position of the
+ *   spin's bit pattern in the ascending list of N_s-bit numbers with N_s bits set.
+ *   The state vector is therefore a row-major dim_up x dim_dn matrix V
+ *   (Fig. 2) and
+ *       H v = (H_up (x) I) v + (I (x) H_dn) v + U popcount(up & dn) o v
+ *   (eq. 14; Algorithms 2-4), fused with the
+ *   Lanczos updates of Algorithm 1 in its two-vector form
+ *   (eq. 12-13).
+ *
+ * Conventions
+ *   - All functions return 0 (HUBBARD_OK) or a negative error code; nothing
+ *     throws, aborts or keeps global state.  hubbard_strerror() names a code.
+ *   - "host" pointers are ordinary CPU memory, "device" pointers are CUDA
+ *     device memory of the current device; the caller owns every buffer it
+ *     passes in.  The model owns its tables and its Lanczos work vectors.
+ *   - dtype: HUBBARD_F32 (0) or HUBBARD_F64 (1) is the storage AND arithmetic
+ *     type of state vectors; alpha/beta and all reductions are double.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default
+ *     stream).
+ *   - There is no CPU fallback: every compute call needs a CUDA device and
+ *     fails with HUBBARD_ERR_CUDA / HUBBARD_ERR_NO_DEVICE otherwise.
+ */
+#ifndef HUBBARD_B200_H
+#define HUBBARD_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct hubbard_model hubbard_model;
+
+enum {
+    HUBBARD_F32 = 0,
+    HUBBARD_F64 = 1
+};
+
+enum {
+    HUBBARD_OK = 0,
+    HUBBARD_ERR_INVALID = -1,    /* bad argument (range, null pointer, aliasing) */
+    HUBBARD_ERR_HOST_OOM = -2,   /* host allocation failed */
+    HUBBARD_ERR_DEVICE_OOM = -3, /* cudaMalloc failed */
+    HUBBARD_ERR_CUDA = -4,       /* any other CUDA error; see hubbard_last_cuda_error */
+    HUBBARD_ERR_NO_DEVICE = -5,  /* model was made by hubbard_create_host: no device state */
+    HUBBARD_ERR_UNSUPPORTED = -6 /* sector too large for the index types used */
+};
+
+/* Kernel variants selectable with hubbard_set_variant (for measurement; every
+ * variant computes the same H v). */
+enum {
+    HUBBARD_VARIANT_AUTO = 0,    /* library picks per model (default) */
+    HUBBARD_VARIANT_PAPER = 1,   /* Algorithms 2-4 restated: one thread per element, one fused kernel */
+    HUBBARD_VARIANT_TWOSWEEP = 2 /* row sweep (down term + diagonal, row staged in shared memory)
+                                    + strip sweep (up term over L2-resident column strips) */
+};
+
+/* ---- construction ("first, we prepare the data on the host") ----
+ *
+ * hubbard_create: enumerate both spin sectors, build the
+ * per-spin hopping tables with fermionic signs (eq. 9-10;
+ * element = -t * (-1)^(same-spin electrons on sites strictly between the two
+ * ends of the bond)), upload them, and return a model in *out.
+ *   n_sites  1..32       number of lattice sites N_s (site k = bit k)
+ *   n_up,n_dn 0..n_sites electrons per spin
+ *   bonds    host array of 2*n_bonds site ids: undirected neighbour pairs, each
+ *            listed once; both hop directions are generated ("+ h.c.").  A pair
+ *            listed twice adds (effective 2t).  i == j is invalid.
+ *   t, U     couplings of eq. (2)
+ *   dtype    HUBBARD_F32 / HUBBARD_F64
+ * Errors: INVALID (ranges, null), UNSUPPORTED (dim_up or dim_dn >= 2^31 - 1),
+ * HOST_OOM, DEVICE_OOM, CUDA.  On error *out is NULL.
+ *
+ * hubbard_create_host: the host half only (basis + tables, no CUDA call) for
+ * inspection with hubbard_get_basis / hubbard_get_hops on a machine without a
+ * GPU; compute calls on such a model return HUBBARD_ERR_NO_DEVICE.
+ */
+int hubbard_create(hubbard_model **out, int n_sites, int n_up, int n_dn,
+                   const int32_t *bonds, int n_bonds, double t, double U, int dtype);
+int hubbard_create_host(hubbard_model **out, int n_sites, int n_up, int n_dn,
+                        const int32_t *bonds, int n_bonds, double t, double U, int dtype);
+
+/* Frees tables, work vectors and the model itself.  NULL is allowed. */
+void hubbard_destroy(hubbard_model *m);
+
+/* dim_up = C(N_s,N_up), dim_dn = C(N_s,N_dn) (eq. 5);
+ * dim = dim_up*dim_dn may exceed 2^31.  Either output pointer may be NULL. */
+int hubbard_dims(const hubbard_model *m, int64_t *dim_up, int64_t *dim_dn);
+
+/* Change U without rebuilding tables (the diagonal is never stored,
+ * PAPER.md:198,303-317). */
+int hubbard_set_U(hubbard_model *m, double U);
+
+/* Select the kernel variant (HUBBARD_VARIANT_*). */
+int hubbard_set_variant(hubbard_model *m, int variant);
+
+/* ---- the hot path ----
+ *
+ * hubbard_apply: y = H x.  x_dev, y_dev: device arrays of
+ * dim elements of the model's dtype, element J = i_up*dim_dn + i_dn (eq. 7),
+ * 16-byte aligned, not aliased (INVALID if x_dev == y_dev).  Enqueued on
+ * `stream`; returns without synchronising.
+ */
+int hubbard_apply(hubbard_model *m, const void *x_dev, void *y_dev, void *stream);
+
+/* lanczos_run: Algorithm 1 with the two-vector update of
+ * eq. 13, H f_j fused with "- b_j f_{j-1}" and the a_j dot
+ * product, "q - a_j f_j" fused with the b_{j+1} norm; normalisation is carried
+ * as a scalar into the next iteration.
+ *   v0_dev      device, dim elements of the model's dtype: start vector f_1; need
+ *               not be normalised; not modified.
+ *   iters       number of iterations m requested (>= 0)
+ *   alpha_host  host, iters doubles: alpha_host[j] = a_{j+1}
+ *   beta_host   host, iters doubles: beta_host[j]  = b_{j+2}
+ *               (T_m of PAPER.md:150 = diag alpha[0..m-1], off-diag beta[0..m-2])
+ *   iters_done  host, may be NULL: iterations completed; < iters on breakdown
+ *               (Algorithm 1 lines 8-10, read as b_{j+1} <= tau*max(1,max_k|a_k|)
+ *               or not finite, tau = 1e-10 for f64 / 1e-5 for f32; see
+ *               lanczos_set_tau).
+ * Work vectors (2 * dim elements) are allocated on first use and kept.
+ * The call enqueues everything on `stream`, then synchronises it and fills the
+ * host arrays.  Errors: INVALID, DEVICE_OOM, CUDA, NO_DEVICE.
+ */
+int lanczos_run(hubbard_model *m, const void *v0_dev, int iters,
+                double *alpha_host, double *beta_host, int *iters_done, void *stream);
+
+/* Breakdown threshold tau (>= 0; 0 = the paper's literal "b = 0" test). */
+int lanczos_set_tau(hubbard_model *m, double tau);
+
+/* ---- same calls with HOST vectors (copies inside): the end-to-end entry ----
+ * x_host/y_host/v0_host: host arrays of dim elements of the model's dtype.
+ * The library stages them through its own device buffers (allocated on first
+ * use, kept), runs the device path above on `stream`, copies the result back
+ * and synchronises. */
+int hubbard_apply_host(hubbard_model *m, const void *x_host, void *y_host, void *stream);
+int lanczos_run_host(hubbard_model *m, const void *v0_host, int iters,
+                     double *alpha_host, double *beta_host, int *iters_done, void *stream);
+
+/* ---- introspection for bit-exact table parity ----
+ *
+ * hubbard_get_basis: states_host[i] = i-th bit pattern of spin `spin`
+ * (0 = up, 1 = down), dim_spin entries, ascending.
+ *
+ * hubbard_get_hops: the per-spin hopping matrix H_spin of eq. 14 in canonical
+ * ELL form, independent of the device layout: row-major dim_spin x width,
+ * entries of a row sorted by ascending column, duplicates merged, exact zeros
+ * dropped, padding col = -1 / val = 0 (PAPER.md:208-230 describes ELL; the
+ * paper pads with 0).  Call with cols_host == NULL to obtain only *width
+ * (= max nonzeros per row).
+ */
+int hubbard_get_basis(const hubbard_model *m, int spin, uint32_t *states_host);
+int hubbard_get_hops(const hubbard_model *m, int spin, int *width,
+                     int32_t *cols_host, double *vals_host);
+
+/* ---- host utility, off the hot path ----
+ * e0 = smallest eigenvalue of the symmetric tridiagonal T_m with diagonal
+ * alpha[0..m-1] and off-diagonal beta[0..m-2]; m >= 1. */
+int lanczos_ground_energy(const double *alpha, const double *beta, int m, double *e0);
+
+/* ---- measurement hooks ----
+ * hubbard_profile(m, 1) makes every later kernel launch of this model be
+ * bracketed by CUDA events on its stream; hubbard_kernel_times then returns,
+ * per kernel class, the number of launches and the summed device time in ms
+ * since the last hubbard_profile call (it synchronises the recorded events).
+ * Classes: 0 = H v kernel(s) of variant PAPER, 1 = row sweep, 2 = strip sweep,
+ * 3 = Lanczos axpy+norm sweep, 4 = scalar/finalise kernels, 5 = setup (copy,
+ * initial norm).  Arrays have HUBBARD_N_KCLASS entries.
+ * hubbard_launch_count: kernels launched by this model since creation. */
+#define HUBBARD_N_KCLASS 6
+int hubbard_profile(hubbard_model *m, int enable);
+int hubbard_kernel_times(hubbard_model *m, int64_t *launches, double *ms);
+int64_t hubbard_launch_count(const hubbard_model *m);
+
+/* Last CUDA error code (cudaError_t as int) seen by this model, 0 if none. */
+int hubbard_last_cuda_error(const hubbard_model *m);
+const char *hubbard_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HUBBARD_B200_H */

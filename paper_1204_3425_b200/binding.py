@@ -1,0 +1,235 @@
+"""Thin ctypes binding of libhubbard_b200 (include/hubbard.h).  Argument
+marshalling only: every step of the path runs in the library's CUDA kernels.
+Function names are those of the C ABI.  There is no fallback: if the library
+cannot be loaded, importing this module raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from pathlib import Path
+
+import numpy as np
+
+from . import build as _build
+
+HUBBARD_F32, HUBBARD_F64 = 0, 1
+VARIANT_AUTO, VARIANT_PAPER, VARIANT_TWOSWEEP = 0, 1, 2
+N_KCLASS = 6
+KCLASS_NAMES = ("hv_paper", "row_sweep", "strip_sweep", "axpy_norm", "scalar", "setup")
+
+ABI_SYMBOLS = (
+    "hubbard_create", "hubbard_create_host", "hubbard_destroy", "hubbard_dims", "hubbard_set_U",
+    "hubbard_set_variant", "hubbard_apply", "lanczos_run", "lanczos_set_tau", "hubbard_apply_host",
+    "lanczos_run_host", "hubbard_get_basis", "hubbard_get_hops", "lanczos_ground_energy",
+    "hubbard_profile", "hubbard_kernel_times", "hubbard_launch_count", "hubbard_last_cuda_error",
+    "hubbard_strerror",
+)
+
+
+def _load() -> C.CDLL:
+    path: Path = _build.LIB
+    if not path.exists():
+        path = _build.build()
+    lib = C.CDLL(str(path))
+    vp, i32, i64, dbl = C.c_void_p, C.c_int, C.c_int64, C.c_double
+    P = C.POINTER
+    lib.hubbard_create.argtypes = [P(vp), i32, i32, i32, P(C.c_int32), i32, dbl, dbl, i32]
+    lib.hubbard_create_host.argtypes = lib.hubbard_create.argtypes
+    lib.hubbard_destroy.argtypes = [vp]
+    lib.hubbard_destroy.restype = None
+    lib.hubbard_dims.argtypes = [vp, P(i64), P(i64)]
+    lib.hubbard_set_U.argtypes = [vp, dbl]
+    lib.hubbard_set_variant.argtypes = [vp, i32]
+    lib.hubbard_apply.argtypes = [vp, vp, vp, vp]
+    lib.lanczos_run.argtypes = [vp, vp, i32, P(dbl), P(dbl), P(i32), vp]
+    lib.lanczos_set_tau.argtypes = [vp, dbl]
+    lib.hubbard_apply_host.argtypes = [vp, vp, vp, vp]
+    lib.lanczos_run_host.argtypes = [vp, vp, i32, P(dbl), P(dbl), P(i32), vp]
+    lib.hubbard_get_basis.argtypes = [vp, i32, P(C.c_uint32)]
+    lib.hubbard_get_hops.argtypes = [vp, i32, P(i32), P(C.c_int32), P(dbl)]
+    lib.lanczos_ground_energy.argtypes = [P(dbl), P(dbl), i32, P(dbl)]
+    lib.hubbard_profile.argtypes = [vp, i32]
+    lib.hubbard_kernel_times.argtypes = [vp, P(i64), P(dbl)]
+    lib.hubbard_launch_count.argtypes = [vp]
+    lib.hubbard_launch_count.restype = i64
+    lib.hubbard_last_cuda_error.argtypes = [vp]
+    lib.hubbard_strerror.argtypes = [i32]
+    lib.hubbard_strerror.restype = C.c_char_p
+    return lib
+
+
+lib = _load()
+LIB_PATH = str(_build.LIB)
+
+
+class HubbardError(RuntimeError):
+    def __init__(self, code: int, what: str, cuda: int = 0):
+        self.code = code
+        msg = f"{what}: {lib.hubbard_strerror(code).decode()} ({code})"
+        if cuda:
+            msg += f" [cudaError {cuda}]"
+        super().__init__(msg)
+
+
+def _check(code: int, what: str, handle=None):
+    if code != 0:
+        raise HubbardError(code, what, lib.hubbard_last_cuda_error(handle) if handle else 0)
+
+
+def _bonds_array(bonds) -> np.ndarray:
+    return np.ascontiguousarray(np.array(list(bonds), dtype=np.int32).reshape(-1, 2))
+
+
+def _dtype_code(dtype) -> int:
+    s = str(dtype)
+    if s in ("f32", "float32", "torch.float32", "0"):
+        return HUBBARD_F32
+    if s in ("f64", "float64", "torch.float64", "1"):
+        return HUBBARD_F64
+    raise ValueError(f"dtype {dtype!r}: use 'f32' or 'f64'")
+
+
+def _dptr(t) -> int:
+    """Device pointer of a contiguous CUDA torch tensor."""
+    if not t.is_cuda or not t.is_contiguous():
+        raise ValueError("expected a contiguous CUDA tensor")
+    return t.data_ptr()
+
+
+def _stream(stream) -> int:
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+    return getattr(stream, "cuda_stream", stream)
+
+
+class Model:
+    """Owner of a `hubbard_model*`; methods are the ABI calls of the same name."""
+
+    def __init__(self, n_sites, n_up, n_dn, bonds, t, U, dtype="f64", host_only=False):
+        self._h = C.c_void_p()
+        b = _bonds_array(bonds)
+        fn = lib.hubbard_create_host if host_only else lib.hubbard_create
+        code = fn(C.byref(self._h), n_sites, n_up, n_dn, b.ctypes.data_as(C.POINTER(C.c_int32)), len(b),
+                  float(t), float(U), _dtype_code(dtype))
+        _check(code, "hubbard_create_host" if host_only else "hubbard_create")
+        self.dtype_code = _dtype_code(dtype)
+        du, dd = C.c_int64(), C.c_int64()
+        _check(lib.hubbard_dims(self._h, C.byref(du), C.byref(dd)), "hubbard_dims")
+        self.dim_up, self.dim_dn = du.value, dd.value
+        self.dim = self.dim_up * self.dim_dn
+
+    # -- lifetime
+    def hubbard_destroy(self):
+        if self._h:
+            lib.hubbard_destroy(self._h)
+            self._h = C.c_void_p()
+
+    close = hubbard_destroy
+
+    def __del__(self):
+        try:
+            self.hubbard_destroy()
+        except Exception:
+            pass
+
+    # -- configuration
+    def hubbard_set_U(self, U):
+        _check(lib.hubbard_set_U(self._h, float(U)), "hubbard_set_U")
+
+    def hubbard_set_variant(self, variant):
+        _check(lib.hubbard_set_variant(self._h, int(variant)), "hubbard_set_variant")
+
+    def lanczos_set_tau(self, tau):
+        _check(lib.lanczos_set_tau(self._h, float(tau)), "lanczos_set_tau")
+
+    # -- hot path, device buffers (torch CUDA tensors)
+    def hubbard_apply(self, x, y, stream=None):
+        _check(lib.hubbard_apply(self._h, _dptr(x), _dptr(y), _stream(stream)), "hubbard_apply", self._h)
+        return y
+
+    def lanczos_run(self, v0, iters, stream=None):
+        alpha = np.zeros(max(iters, 1))
+        beta = np.zeros(max(iters, 1))
+        done = C.c_int(0)
+        dp = C.POINTER(C.c_double)
+        _check(lib.lanczos_run(self._h, _dptr(v0), iters, alpha.ctypes.data_as(dp), beta.ctypes.data_as(dp),
+                               C.byref(done), _stream(stream)), "lanczos_run", self._h)
+        return alpha[:done.value].copy(), beta[:done.value].copy()
+
+    # -- hot path, host buffers (numpy arrays or CPU torch tensors)
+    @staticmethod
+    def _hptr(a) -> int:
+        if isinstance(a, np.ndarray):
+            if not a.flags.c_contiguous:
+                raise ValueError("expected a C-contiguous array")
+            return a.ctypes.data
+        return a.data_ptr()
+
+    def hubbard_apply_host(self, x, y, stream=None):
+        _check(lib.hubbard_apply_host(self._h, self._hptr(x), self._hptr(y), _stream(stream)),
+               "hubbard_apply_host", self._h)
+        return y
+
+    def lanczos_run_host(self, v0, iters, stream=None):
+        alpha = np.zeros(max(iters, 1))
+        beta = np.zeros(max(iters, 1))
+        done = C.c_int(0)
+        dp = C.POINTER(C.c_double)
+        _check(lib.lanczos_run_host(self._h, self._hptr(v0), iters, alpha.ctypes.data_as(dp),
+                                    beta.ctypes.data_as(dp), C.byref(done), _stream(stream)),
+               "lanczos_run_host", self._h)
+        return alpha[:done.value].copy(), beta[:done.value].copy()
+
+    # -- introspection
+    def hubbard_get_basis(self, spin):
+        n = self.dim_up if spin == 0 else self.dim_dn
+        out = np.empty(n, dtype=np.uint32)
+        _check(lib.hubbard_get_basis(self._h, spin, out.ctypes.data_as(C.POINTER(C.c_uint32))), "hubbard_get_basis")
+        return out
+
+    def hubbard_get_hops(self, spin):
+        n = self.dim_up if spin == 0 else self.dim_dn
+        w = C.c_int(0)
+        _check(lib.hubbard_get_hops(self._h, spin, C.byref(w), None, None), "hubbard_get_hops")
+        cols = np.empty((n, w.value), dtype=np.int32)
+        vals = np.empty((n, w.value), dtype=np.float64)
+        _check(lib.hubbard_get_hops(self._h, spin, C.byref(w), cols.ctypes.data_as(C.POINTER(C.c_int32)),
+                                    vals.ctypes.data_as(C.POINTER(C.c_double))), "hubbard_get_hops")
+        return w.value, cols, vals
+
+    # -- measurement hooks
+    def hubbard_profile(self, enable=True):
+        _check(lib.hubbard_profile(self._h, int(bool(enable))), "hubbard_profile")
+
+    def hubbard_kernel_times(self):
+        n = (C.c_int64 * N_KCLASS)()
+        ms = (C.c_double * N_KCLASS)()
+        _check(lib.hubbard_kernel_times(self._h, n, ms), "hubbard_kernel_times", self._h)
+        return {KCLASS_NAMES[k]: (int(n[k]), float(ms[k])) for k in range(N_KCLASS)}
+
+    def hubbard_launch_count(self):
+        return int(lib.hubbard_launch_count(self._h))
+
+
+def hubbard_create(n_sites, n_up, n_dn, bonds, t, U, dtype="f64") -> Model:
+    return Model(n_sites, n_up, n_dn, bonds, t, U, dtype)
+
+
+def hubbard_create_host(n_sites, n_up, n_dn, bonds, t, U, dtype="f64") -> Model:
+    return Model(n_sites, n_up, n_dn, bonds, t, U, dtype, host_only=True)
+
+
+def lanczos_ground_energy(alpha, beta, m=None) -> float:
+    a = np.ascontiguousarray(alpha, dtype=np.float64)
+    b = np.ascontiguousarray(beta, dtype=np.float64)
+    m = len(a) if m is None else int(m)
+    if len(b) < max(m - 1, 0) or len(a) < m:
+        raise ValueError("alpha/beta shorter than m")
+    if len(b) == 0:
+        b = np.zeros(1)
+    e0 = C.c_double(0.0)
+    dp = C.POINTER(C.c_double)
+    _check(lib.lanczos_ground_energy(a.ctypes.data_as(dp), b.ctypes.data_as(dp), m, C.byref(e0)),
+           "lanczos_ground_energy")
+    return e0.value

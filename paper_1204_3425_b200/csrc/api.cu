@@ -1,0 +1,555 @@
+// C ABI of libhubbard_b200 (include/hubbard.h): model construction, table
+// upload, kernel launches.  Nothing here throws across the boundary.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "kernels_lanczos.cuh"
+#include "kernels_paper.cuh"
+#include "kernels_twosweep.cuh"
+#include "model.h"
+
+using namespace hub;
+
+namespace {
+
+#define CU_TRY(m, expr)                                                   \
+    do {                                                                  \
+        cudaError_t e__ = (expr);                                         \
+        if (e__ != cudaSuccess) {                                         \
+            (m)->last_cuda_error = (int)e__;                              \
+            cudaGetLastError();                                           \
+            return (e__ == cudaErrorMemoryAllocation) ? HUBBARD_ERR_DEVICE_OOM : HUBBARD_ERR_CUDA; \
+        }                                                                 \
+    } while (0)
+
+template <typename U>
+int dev_upload(hubbard_model *m, const std::vector<U> &h, const U **out)
+{
+    void *p = nullptr;
+    size_t bytes = std::max<size_t>(h.size(), 1) * sizeof(U);
+    CU_TRY(m, cudaMalloc(&p, bytes));
+    m->dev_allocs.push_back(p);
+    if (!h.empty()) CU_TRY(m, cudaMemcpy(p, h.data(), h.size() * sizeof(U), cudaMemcpyHostToDevice));
+    *out = static_cast<const U *>(p);
+    return HUBBARD_OK;
+}
+
+size_t elem_size(const hubbard_model *m) { return m->dtype == HUBBARD_F32 ? 4 : 8; }
+int64_t model_dim(const hubbard_model *m) { return m->up.dim * m->dn.dim; }
+
+int build_host(hubbard_model **out, int n_sites, int n_up, int n_dn, const int32_t *bonds, int n_bonds,
+               double t, double U, int dtype)
+{
+    if (!out) return HUBBARD_ERR_INVALID;
+    *out = nullptr;
+    if (dtype != HUBBARD_F32 && dtype != HUBBARD_F64) return HUBBARD_ERR_INVALID;
+    if (!std::isfinite(t) || !std::isfinite(U)) return HUBBARD_ERR_INVALID;
+    hubbard_model *m = new (std::nothrow) hubbard_model();
+    if (!m) return HUBBARD_ERR_HOST_OOM;
+    int rc = build_spin_table(n_sites, n_up, bonds, n_bonds, m->up);
+    if (rc == 0) rc = build_spin_table(n_sites, n_dn, bonds, n_bonds, m->dn);
+    if (rc != 0) {
+        delete m;
+        return rc == -1 ? HUBBARD_ERR_INVALID : rc == -2 ? HUBBARD_ERR_HOST_OOM : HUBBARD_ERR_UNSUPPORTED;
+    }
+    m->n_sites = n_sites; m->n_up = n_up; m->n_dn = n_dn; m->dtype = dtype; m->t = t; m->U = U;
+    try {
+        m->bonds.assign(bonds, bonds + 2 * (size_t)n_bonds);
+    } catch (const std::bad_alloc &) {
+        delete m;
+        return HUBBARD_ERR_HOST_OOM;
+    }
+    *out = m;
+    return HUBBARD_OK;
+}
+
+// Device layouts of the two hop tables (see model.h / DESIGN.md "data layout").
+int upload_tables(hubbard_model *m)
+{
+    DevModel &D = m->dev;
+    D.dim_up = m->up.dim; D.dim_dn = m->dn.dim; D.t = m->t; D.U = m->U;
+    int rc;
+    if ((rc = dev_upload(m, m->up.states, &D.st_up))) return rc;
+    if ((rc = dev_upload(m, m->dn.states, &D.st_dn))) return rc;
+    try {
+        // up: row-major ELL
+        D.w_up = std::max(m->up.width, 1);
+        std::vector<uint32_t> ue((size_t)m->up.dim * D.w_up, kPadEntry);
+        std::vector<int32_t> uc((size_t)m->up.dim);
+        for (int64_t r = 0; r < m->up.dim; ++r) {
+            int n = (int)(m->up.rowptr[r + 1] - m->up.rowptr[r]);
+            uc[(size_t)r] = n;
+            for (int k = 0; k < n; ++k) {
+                size_t s = (size_t)(m->up.rowptr[r] + k);
+                ue[(size_t)r * D.w_up + k] = (uint32_t)m->up.col[s] * 2u + m->up.plus[s];
+            }
+        }
+        if ((rc = dev_upload(m, ue, &D.up_ent))) return rc;
+        if ((rc = dev_upload(m, uc, &D.up_cnt))) return rc;
+        // down: column-major ELL, padded with the zero slot col = dim_dn
+        D.w_dn = std::max(m->dn.width, 1);
+        D.ld_dn = (m->dn.dim + 31) / 32 * 32;
+        const uint32_t pad = (uint32_t)m->dn.dim * 2u;
+        std::vector<uint32_t> de((size_t)D.ld_dn * D.w_dn, pad);
+        std::vector<int32_t> dc((size_t)m->dn.dim);
+        for (int64_t r = 0; r < m->dn.dim; ++r) {
+            int n = (int)(m->dn.rowptr[r + 1] - m->dn.rowptr[r]);
+            dc[(size_t)r] = n;
+            for (int k = 0; k < n; ++k) {
+                size_t s = (size_t)(m->dn.rowptr[r] + k);
+                de[(size_t)k * D.ld_dn + r] = (uint32_t)m->dn.col[s] * 2u + m->dn.plus[s];
+            }
+        }
+        if ((rc = dev_upload(m, de, &D.dn_ent32))) return rc;
+        if ((rc = dev_upload(m, dc, &D.dn_cnt))) return rc;
+        D.dn_ent16 = nullptr;
+        if (m->dn.dim + 1 <= 32768) {
+            std::vector<uint16_t> d16(de.size());
+            for (size_t i = 0; i < de.size(); ++i) d16[i] = (uint16_t)de[i];
+            if ((rc = dev_upload(m, d16, &D.dn_ent16))) return rc;
+        }
+    } catch (const std::bad_alloc &) {
+        return HUBBARD_ERR_HOST_OOM;
+    }
+    return HUBBARD_OK;
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------ launches
+namespace {
+
+struct ProfScope {
+    hubbard_model *m;
+    cudaStream_t st;
+    ProfRecord rec{};
+    bool on;
+    ProfScope(hubbard_model *m_, int kclass, cudaStream_t st_) : m(m_), st(st_), on(m_->profiling)
+    {
+        if (!on) return;
+        rec.kclass = kclass;
+        if (cudaEventCreate(&rec.e0) != cudaSuccess || cudaEventCreate(&rec.e1) != cudaSuccess) { on = false; return; }
+        cudaEventRecord(rec.e0, st);
+    }
+    ~ProfScope()
+    {
+        if (!on) return;
+        cudaEventRecord(rec.e1, st);
+        m->prof.push_back(rec);
+    }
+};
+
+int after_launch(hubbard_model *m)
+{
+    ++m->launches;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) {
+        m->last_cuda_error = (int)e;
+        return HUBBARD_ERR_CUDA;
+    }
+    return HUBBARD_OK;
+}
+
+int env_int(const char *name, int dflt)
+{
+    const char *v = getenv(name);
+    if (!v || !*v) return dflt;
+    return atoi(v);
+}
+
+int ensure_partials(hubbard_model *m, int64_t n)
+{
+    if (n <= m->n_partial) return HUBBARD_OK;
+    if (m->d_partial) cudaFree(m->d_partial);
+    m->d_partial = nullptr;
+    m->n_partial = 0;
+    CU_TRY(m, cudaMalloc((void **)&m->d_partial, (size_t)n * sizeof(double)));
+    m->n_partial = n;
+    return HUBBARD_OK;
+}
+
+int resolve_variant(const hubbard_model *m)
+{
+    if (m->variant != HUBBARD_VARIANT_AUTO) return m->variant;
+    return (m->dn.dim >= 512) ? HUBBARD_VARIANT_TWOSWEEP : HUBBARD_VARIANT_PAPER;
+}
+
+// ---- variant PAPER
+template <typename T, bool LZ>
+int launch_paper(hubbard_model *m, const T *x, T *y, cudaStream_t st)
+{
+    const DevModel &D = m->dev;
+    int64_t bps = (D.dim_dn + kPaperThreads - 1) / kPaperThreads;
+    int64_t gy = std::min<int64_t>(D.dim_up, 65535);
+    if (LZ) gy = std::max<int64_t>(1, std::min<int64_t>(gy, (1 << 16) / bps));
+    if (bps > 0x7fffffff) return HUBBARD_ERR_UNSUPPORTED;
+    SweepArgs<T> A{x, y, LZ ? m->d_scal : nullptr, m->d_partial};
+    if (LZ) { int rc = ensure_partials(m, bps * gy); if (rc) return rc; A.partials = m->d_partial; }
+    ProfScope ps(m, 0, st);
+    hv_paper_kernel<T, LZ><<<dim3((unsigned)bps, (unsigned)gy), kPaperThreads, (size_t)D.w_up * 4, st>>>(D, A);
+    return after_launch(m);
+}
+
+// ---- variant TWOSWEEP
+template <typename T, typename E, int R, bool LZ>
+int launch_row_staged(hubbard_model *m, const SweepArgs<T> &A, const E *ent, size_t smem, cudaStream_t st)
+{
+    auto kern = row_sweep_kernel<T, E, R, LZ>;
+    CU_TRY(m, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int per_sm = std::max(1, std::min(2, (int)((size_t)m->max_smem_optin / (smem + 1024))));
+    int64_t groups = (m->dev.dim_up + R - 1) / R;
+    int grid = (int)std::min<int64_t>(groups, (int64_t)m->sm_count * per_sm);
+    ProfScope ps(m, 1, st);
+    kern<<<grid, kRowThreads, smem, st>>>(m->dev, A, ent);
+    return after_launch(m);
+}
+
+template <typename T, typename E, bool LZ>
+int launch_row(hubbard_model *m, const SweepArgs<T> &A, const E *ent, cudaStream_t st)
+{
+    const DevModel &D = m->dev;
+    constexpr int N = 16 / sizeof(T);
+    auto need = [&](int R) { return ((size_t)R * D.dim_dn + N) * sizeof(T); };
+    int R = env_int("HUBBARD_ROW_R", 0);
+    if (R == 0) {
+        // default: the largest R in {4,2,1} that still lets two CTAs share an SM, else R = 1
+        R = 1;
+        for (int r : {4, 2})
+            if (need(r) + 1024 <= (size_t)m->max_smem_optin / 2) { R = r; break; }
+    }
+    if (R != 1 && R != 2 && R != 4) R = 1;
+    while (R > 1 && need(R) > (size_t)m->max_smem_optin) R >>= 1;
+    if (need(R) > (size_t)m->max_smem_optin) {
+        int64_t bps = (D.dim_dn + kPaperThreads - 1) / kPaperThreads;
+        int64_t gy = std::min<int64_t>(D.dim_up, 65535);
+        ProfScope ps(m, 1, st);
+        row_sweep_direct_kernel<T, E, LZ><<<dim3((unsigned)bps, (unsigned)gy), kPaperThreads, 0, st>>>(D, A, ent);
+        return after_launch(m);
+    }
+    switch (R) {
+        case 4: return launch_row_staged<T, E, 4, LZ>(m, A, ent, need(4), st);
+        case 2: return launch_row_staged<T, E, 2, LZ>(m, A, ent, need(2), st);
+        default: return launch_row_staged<T, E, 1, LZ>(m, A, ent, need(1), st);
+    }
+}
+
+template <typename T, bool LZ>
+int launch_strip(hubbard_model *m, SweepArgs<T> A, cudaStream_t st)
+{
+    const DevModel &D = m->dev;
+    constexpr int N = 16 / sizeof(T);
+    int VW = N;
+    while (VW > 1 && (D.dim_dn % VW) != 0) VW >>= 1;
+    StripPlan P;
+    double mb = (double)env_int("HUBBARD_STRIP_MB", 24);
+    int64_t W = (int64_t)(mb * 1048576.0 / ((double)D.dim_up * sizeof(T)));
+    W = std::max<int64_t>(32, W / 32 * 32);
+    int64_t dd_up = (D.dim_dn + VW - 1) / VW * VW;
+    W = std::min(W, dd_up);
+    P.W = W;
+    P.n_strips = (D.dim_dn + W - 1) / W;
+    int RB = env_int("HUBBARD_STRIP_RB", 0);
+    if (RB <= 0) RB = (int)std::max<int64_t>(8, (2048 * (int64_t)VW + W - 1) / W);
+    RB = (int)std::min<int64_t>(RB, D.dim_up);
+    P.RB = RB;
+    P.bps = (D.dim_up + RB - 1) / RB;
+    int64_t nb = P.n_strips * P.bps;
+    if (nb > 0x7fffffff) return HUBBARD_ERR_UNSUPPORTED;
+    if (LZ) { int rc = ensure_partials(m, nb); if (rc) return rc; A.partials = m->d_partial; }
+    size_t smem = (size_t)RB * (D.w_up + 1) * 4;
+    ProfScope ps(m, 2, st);
+    if (VW == 4) {
+        if constexpr (sizeof(T) == 4) strip_sweep_kernel<T, 4, LZ><<<(unsigned)nb, kStripThreads, smem, st>>>(D, A, P);
+    } else if (VW == 2) {
+        strip_sweep_kernel<T, 2, LZ><<<(unsigned)nb, kStripThreads, smem, st>>>(D, A, P);
+    } else {
+        strip_sweep_kernel<T, 1, LZ><<<(unsigned)nb, kStripThreads, smem, st>>>(D, A, P);
+    }
+    return after_launch(m);
+}
+
+// y = H x (LZ = false) or the fused Lanczos H f_j - b_j f_{j-1}, a_j (LZ = true)
+template <typename T, bool LZ>
+int apply_impl(hubbard_model *m, const T *x, T *y, cudaStream_t st)
+{
+    m->dev.U = m->U;
+    if (resolve_variant(m) == HUBBARD_VARIANT_PAPER) return launch_paper<T, LZ>(m, x, y, st);
+    SweepArgs<T> A{x, y, LZ ? m->d_scal : nullptr, m->d_partial};
+    int rc = m->dev.dn_ent16 ? launch_row<T, uint16_t, LZ>(m, A, m->dev.dn_ent16, st)
+                             : launch_row<T, uint32_t, LZ>(m, A, m->dev.dn_ent32, st);
+    if (rc) return rc;
+    return launch_strip<T, LZ>(m, A, st);
+}
+
+}  // namespace
+
+// --------------------------------------------------------------- Lanczos run
+namespace {
+
+int ensure_lanczos_state(hubbard_model *m, int iters)
+{
+    const size_t bytes = (size_t)model_dim(m) * elem_size(m);
+    for (int i = 0; i < 2; ++i)
+        if (!m->work[i]) CU_TRY(m, cudaMalloc(&m->work[i], std::max<size_t>(bytes, 16)));
+    if (!m->d_scal) CU_TRY(m, cudaMalloc((void **)&m->d_scal, sizeof(LanczosScalars)));
+    if (iters > m->coef_cap) {
+        if (m->d_alpha) cudaFree(m->d_alpha);
+        if (m->d_beta) cudaFree(m->d_beta);
+        m->d_alpha = m->d_beta = nullptr;
+        m->coef_cap = 0;
+        CU_TRY(m, cudaMalloc((void **)&m->d_alpha, (size_t)iters * sizeof(double)));
+        CU_TRY(m, cudaMalloc((void **)&m->d_beta, (size_t)iters * sizeof(double)));
+        m->coef_cap = iters;
+    }
+    return HUBBARD_OK;
+}
+
+template <typename T>
+int lanczos_impl(hubbard_model *m, const T *v0, int iters, double *alpha, double *beta, int *done, cudaStream_t st)
+{
+    const int64_t dim = model_dim(m);
+    int rc = ensure_lanczos_state(m, iters);
+    if (rc) return rc;
+    const int vec_grid = (int)std::max<int64_t>(1, std::min<int64_t>((int64_t)m->sm_count * 4, (dim + 2047) / 2048));
+    if ((rc = ensure_partials(m, vec_grid))) return rc;
+    T *cur = static_cast<T *>(m->work[0]), *prev = static_cast<T *>(m->work[1]);
+    const double tau = m->tau >= 0 ? m->tau : (m->dtype == HUBBARD_F64 ? 1e-10 : 1e-5);
+    {
+        ProfScope ps(m, 5, st);
+        CU_TRY(m, cudaMemcpyAsync(cur, v0, (size_t)dim * sizeof(T), cudaMemcpyDeviceToDevice, st));
+        CU_TRY(m, cudaMemsetAsync(prev, 0, (size_t)dim * sizeof(T), st));   // line 2: f_0 <- 0
+        CU_TRY(m, cudaMemsetAsync(m->d_scal, 0, sizeof(LanczosScalars), st));
+        lanczos_init_kernel<T><<<vec_grid, kVecThreads, 0, st>>>(cur, dim, m->d_scal, m->d_partial, tau);
+        if ((rc = after_launch(m))) return rc;
+    }
+    for (int j = 0; j < iters; ++j) {
+        if ((rc = apply_impl<T, true>(m, cur, prev, st))) return rc;     // lines 4-5 (+ eq. 13)
+        if ((rc = ensure_partials(m, vec_grid))) return rc;
+        {
+            ProfScope ps(m, 3, st);
+            lanczos_axpy_norm_kernel<T><<<vec_grid, kVecThreads, 0, st>>>(cur, prev, dim, m->d_scal, m->d_partial,
+                                                                         m->d_alpha, m->d_beta);   // lines 6-11
+            if ((rc = after_launch(m))) return rc;
+        }
+        std::swap(cur, prev);
+    }
+    LanczosScalars h{};
+    CU_TRY(m, cudaMemcpyAsync(&h, m->d_scal, sizeof(h), cudaMemcpyDeviceToHost, st));
+    CU_TRY(m, cudaStreamSynchronize(st));
+    int n = std::max(0, std::min(h.j, iters));
+    if (n > 0) {
+        CU_TRY(m, cudaMemcpy(alpha, m->d_alpha, (size_t)n * sizeof(double), cudaMemcpyDeviceToHost));
+        CU_TRY(m, cudaMemcpy(beta, m->d_beta, (size_t)n * sizeof(double), cudaMemcpyDeviceToHost));
+    }
+    if (done) *done = n;
+    return HUBBARD_OK;
+}
+
+int ensure_stage(hubbard_model *m, int which)
+{
+    if (m->stage[which]) return HUBBARD_OK;
+    CU_TRY(m, cudaMalloc(&m->stage[which], std::max<size_t>((size_t)model_dim(m) * elem_size(m), 16)));
+    return HUBBARD_OK;
+}
+
+int check_device_model(const hubbard_model *m)
+{
+    if (!m) return HUBBARD_ERR_INVALID;
+    if (!m->has_device) return HUBBARD_ERR_NO_DEVICE;
+    return HUBBARD_OK;
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------ the ABI
+extern "C" {
+
+int hubbard_create_host(hubbard_model **out, int n_sites, int n_up, int n_dn, const int32_t *bonds, int n_bonds,
+                        double t, double U, int dtype)
+{
+    return build_host(out, n_sites, n_up, n_dn, bonds, n_bonds, t, U, dtype);
+}
+
+int hubbard_create(hubbard_model **out, int n_sites, int n_up, int n_dn, const int32_t *bonds, int n_bonds,
+                   double t, double U, int dtype)
+{
+    int rc = build_host(out, n_sites, n_up, n_dn, bonds, n_bonds, t, U, dtype);
+    if (rc) return rc;
+    hubbard_model *m = *out;
+    auto fail = [&](int code) { hubbard_destroy(m); *out = nullptr; return code; };
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(HUBBARD_ERR_CUDA); }
+    cudaDeviceGetAttribute(&m->sm_count, cudaDevAttrMultiProcessorCount, dev);
+    cudaDeviceGetAttribute(&m->max_smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    if (m->sm_count <= 0) m->sm_count = 148;
+    rc = upload_tables(m);
+    if (rc) return fail(rc);
+    m->has_device = true;
+    return HUBBARD_OK;
+}
+
+void hubbard_destroy(hubbard_model *m)
+{
+    if (!m) return;
+    for (auto &r : m->prof) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
+    for (void *p : m->dev_allocs) cudaFree(p);
+    for (int i = 0; i < 2; ++i) { if (m->work[i]) cudaFree(m->work[i]); if (m->stage[i]) cudaFree(m->stage[i]); }
+    if (m->d_scal) cudaFree(m->d_scal);
+    if (m->d_partial) cudaFree(m->d_partial);
+    if (m->d_alpha) cudaFree(m->d_alpha);
+    if (m->d_beta) cudaFree(m->d_beta);
+    delete m;
+}
+
+int hubbard_dims(const hubbard_model *m, int64_t *dim_up, int64_t *dim_dn)
+{
+    if (!m) return HUBBARD_ERR_INVALID;
+    if (dim_up) *dim_up = m->up.dim;
+    if (dim_dn) *dim_dn = m->dn.dim;
+    return HUBBARD_OK;
+}
+
+int hubbard_set_U(hubbard_model *m, double U)
+{
+    if (!m || !std::isfinite(U)) return HUBBARD_ERR_INVALID;
+    m->U = U;
+    m->dev.U = U;
+    return HUBBARD_OK;
+}
+
+int hubbard_set_variant(hubbard_model *m, int variant)
+{
+    if (!m || variant < HUBBARD_VARIANT_AUTO || variant > HUBBARD_VARIANT_TWOSWEEP) return HUBBARD_ERR_INVALID;
+    m->variant = variant;
+    return HUBBARD_OK;
+}
+
+int lanczos_set_tau(hubbard_model *m, double tau)
+{
+    if (!m || !(tau >= 0.0)) return HUBBARD_ERR_INVALID;
+    m->tau = tau;
+    return HUBBARD_OK;
+}
+
+int hubbard_apply(hubbard_model *m, const void *x_dev, void *y_dev, void *stream)
+{
+    int rc = check_device_model(m);
+    if (rc) return rc;
+    if (!x_dev || !y_dev || x_dev == y_dev) return HUBBARD_ERR_INVALID;
+    if (((uintptr_t)x_dev | (uintptr_t)y_dev) & 15) return HUBBARD_ERR_INVALID;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (m->dtype == HUBBARD_F32)
+        return apply_impl<float, false>(m, static_cast<const float *>(x_dev), static_cast<float *>(y_dev), st);
+    return apply_impl<double, false>(m, static_cast<const double *>(x_dev), static_cast<double *>(y_dev), st);
+}
+
+int lanczos_run(hubbard_model *m, const void *v0_dev, int iters, double *alpha_host, double *beta_host,
+                int *iters_done, void *stream)
+{
+    int rc = check_device_model(m);
+    if (rc) return rc;
+    if (iters_done) *iters_done = 0;
+    if (!v0_dev || iters < 0 || (iters > 0 && (!alpha_host || !beta_host))) return HUBBARD_ERR_INVALID;
+    if ((uintptr_t)v0_dev & 15) return HUBBARD_ERR_INVALID;
+    if (iters == 0) return HUBBARD_OK;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (m->dtype == HUBBARD_F32)
+        return lanczos_impl<float>(m, static_cast<const float *>(v0_dev), iters, alpha_host, beta_host, iters_done, st);
+    return lanczos_impl<double>(m, static_cast<const double *>(v0_dev), iters, alpha_host, beta_host, iters_done, st);
+}
+
+int hubbard_apply_host(hubbard_model *m, const void *x_host, void *y_host, void *stream)
+{
+    int rc = check_device_model(m);
+    if (rc) return rc;
+    if (!x_host || !y_host) return HUBBARD_ERR_INVALID;
+    if ((rc = ensure_stage(m, 0)) || (rc = ensure_stage(m, 1))) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const size_t bytes = (size_t)model_dim(m) * elem_size(m);
+    CU_TRY(m, cudaMemcpyAsync(m->stage[0], x_host, bytes, cudaMemcpyHostToDevice, st));
+    if ((rc = hubbard_apply(m, m->stage[0], m->stage[1], stream))) return rc;
+    CU_TRY(m, cudaMemcpyAsync(y_host, m->stage[1], bytes, cudaMemcpyDeviceToHost, st));
+    CU_TRY(m, cudaStreamSynchronize(st));
+    return HUBBARD_OK;
+}
+
+int lanczos_run_host(hubbard_model *m, const void *v0_host, int iters, double *alpha_host, double *beta_host,
+                     int *iters_done, void *stream)
+{
+    int rc = check_device_model(m);
+    if (rc) return rc;
+    if (!v0_host) return HUBBARD_ERR_INVALID;
+    if ((rc = ensure_stage(m, 0))) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    CU_TRY(m, cudaMemcpyAsync(m->stage[0], v0_host, (size_t)model_dim(m) * elem_size(m), cudaMemcpyHostToDevice, st));
+    return lanczos_run(m, m->stage[0], iters, alpha_host, beta_host, iters_done, stream);
+}
+
+int hubbard_get_basis(const hubbard_model *m, int spin, uint32_t *states_host)
+{
+    if (!m || !states_host || (spin != 0 && spin != 1)) return HUBBARD_ERR_INVALID;
+    const SpinTable &tab = spin == 0 ? m->up : m->dn;
+    std::memcpy(states_host, tab.states.data(), tab.states.size() * sizeof(uint32_t));
+    return HUBBARD_OK;
+}
+
+int hubbard_get_hops(const hubbard_model *m, int spin, int *width, int32_t *cols_host, double *vals_host)
+{
+    if (!m || (spin != 0 && spin != 1) || (!width && !cols_host)) return HUBBARD_ERR_INVALID;
+    if ((cols_host == nullptr) != (vals_host == nullptr)) return HUBBARD_ERR_INVALID;
+    try {
+        canonical_ell(spin == 0 ? m->up : m->dn, m->t, width, cols_host, vals_host);
+    } catch (const std::bad_alloc &) {
+        return HUBBARD_ERR_HOST_OOM;
+    }
+    return HUBBARD_OK;
+}
+
+int hubbard_profile(hubbard_model *m, int enable)
+{
+    if (!m) return HUBBARD_ERR_INVALID;
+    for (auto &r : m->prof) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
+    m->prof.clear();
+    for (int k = 0; k < HUBBARD_N_KCLASS; ++k) { m->prof_launches[k] = 0; m->prof_ms[k] = 0.0; }
+    m->profiling = enable != 0;
+    return HUBBARD_OK;
+}
+
+int hubbard_kernel_times(hubbard_model *m, int64_t *launches, double *ms)
+{
+    if (!m || !launches || !ms) return HUBBARD_ERR_INVALID;
+    for (auto &r : m->prof) {
+        CU_TRY(m, cudaEventSynchronize(r.e1));
+        float t = 0.f;
+        CU_TRY(m, cudaEventElapsedTime(&t, r.e0, r.e1));
+        m->prof_launches[r.kclass] += 1;
+        m->prof_ms[r.kclass] += (double)t;
+        cudaEventDestroy(r.e0);
+        cudaEventDestroy(r.e1);
+    }
+    m->prof.clear();
+    for (int k = 0; k < HUBBARD_N_KCLASS; ++k) { launches[k] = m->prof_launches[k]; ms[k] = m->prof_ms[k]; }
+    return HUBBARD_OK;
+}
+
+int64_t hubbard_launch_count(const hubbard_model *m) { return m ? m->launches : 0; }
+int hubbard_last_cuda_error(const hubbard_model *m) { return m ? m->last_cuda_error : 0; }
+
+const char *hubbard_strerror(int code)
+{
+    switch (code) {
+        case HUBBARD_OK: return "ok";
+        case HUBBARD_ERR_INVALID: return "invalid argument";
+        case HUBBARD_ERR_HOST_OOM: return "out of host memory";
+        case HUBBARD_ERR_DEVICE_OOM: return "out of device memory";
+        case HUBBARD_ERR_CUDA: return "CUDA error (see hubbard_last_cuda_error)";
+        case HUBBARD_ERR_NO_DEVICE: return "model has no device state (hubbard_create_host)";
+        case HUBBARD_ERR_UNSUPPORTED: return "sector too large for the index types used";
+        default: return "unknown error";
+    }
+}
+
+}  // extern "C"

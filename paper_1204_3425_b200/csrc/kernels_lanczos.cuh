@@ -1,0 +1,117 @@
+// Lanczos vector sweeps (Algorithm 1).  The paper is silent
+// on how these are done; here each is one streaming sweep with a
+// deterministic grid reduction, and the scalar bookkeeping of the iteration
+// (lines 7-11) is done by the last block to arrive, so the host never
+// synchronises inside the loop.
+#pragma once
+#include "kernels_common.cuh"
+
+namespace hub {
+
+constexpr int kVecThreads = 512;
+
+template <typename T> struct Vec16;          // 16-byte vector of T
+template <> struct Vec16<float>  { using type = float4;  static constexpr int n = 4; };
+template <> struct Vec16<double> { using type = double2; static constexpr int n = 2; };
+
+// ||v0||^2, then c_cur = 1/||v0|| (Algorithm 1 "Require: f_1 of norm 1": the
+// caller's vector is normalised by scalar, its copy u_cur is left unscaled).
+template <typename T>
+__global__ void __launch_bounds__(kVecThreads)
+lanczos_init_kernel(const T *__restrict__ u, int64_t dim, LanczosScalars *S, double *partials, double tau)
+{
+    __shared__ double red[32];
+    __shared__ int flag;
+    using V = typename Vec16<T>::type;
+    constexpr int N = Vec16<T>::n;
+    const int64_t nvec = dim / N;
+    const int64_t per = (nvec + gridDim.x - 1) / gridDim.x;
+    const int64_t lo = blockIdx.x * per, hi = min(nvec, lo + per);
+    double acc = 0.0;
+    for (int64_t i = lo + threadIdx.x; i < hi; i += blockDim.x) {
+        V v = reinterpret_cast<const V *>(u)[i];
+        const T *e = reinterpret_cast<const T *>(&v);
+#pragma unroll
+        for (int k = 0; k < N; ++k) acc += (double)e[k] * (double)e[k];
+    }
+    if (blockIdx.x == gridDim.x - 1)
+        for (int64_t i = nvec * N + threadIdx.x; i < dim; i += blockDim.x) acc += (double)u[i] * (double)u[i];
+    double s = block_sum(acc, red);
+    if (publish_and_check_last(s, partials, blockIdx.x, gridDim.x, &S->ticket, &flag)) {
+        double n2 = sum_partials(partials, gridDim.x, red);
+        if (threadIdx.x == 0) {
+            double nrm = sqrt(n2);
+            bool ok = isfinite(nrm) && nrm > 0.0;
+            S->c_cur = ok ? 1.0 / nrm : 0.0;
+            S->c_prev = 0.0;
+            S->beta = 0.0;       // line 1: b_1 <- 0
+            S->alpha = 0.0;
+            S->amax = 0.0;
+            S->tau = tau;
+            S->j = 0;
+            S->stop = ok ? 0 : 1;
+            S->ticket = 0;
+        }
+    }
+}
+
+// Lines 6-11: w <- w - a_j f_j (f_j = c_cur u_cur), b_{j+1} = ||w||; the last
+// block records a_j, b_{j+1}, applies the breakdown rule (reading Q11) and
+// rotates the scalars: f_{j+1} = w / b_{j+1} is carried as c_cur = 1/b_{j+1}.
+template <typename T>
+__global__ void __launch_bounds__(kVecThreads)
+lanczos_axpy_norm_kernel(const T *__restrict__ u, T *__restrict__ w, int64_t dim, LanczosScalars *S,
+                         double *partials, double *alpha_out, double *beta_out)
+{
+    __shared__ double red[32];
+    __shared__ int flag;
+    if (S->stop) return;
+    using V = typename Vec16<T>::type;
+    constexpr int N = Vec16<T>::n;
+    const T ac = (T)(S->alpha * S->c_cur);
+    const int64_t nvec = dim / N;
+    const int64_t per = (nvec + gridDim.x - 1) / gridDim.x;
+    const int64_t lo = blockIdx.x * per, hi = min(nvec, lo + per);
+    double acc = 0.0;
+    for (int64_t i = lo + threadIdx.x; i < hi; i += blockDim.x) {
+        V uv = reinterpret_cast<const V *>(u)[i];
+        V wv = reinterpret_cast<V *>(w)[i];
+        const T *ue = reinterpret_cast<const T *>(&uv);
+        T *we = reinterpret_cast<T *>(&wv);
+#pragma unroll
+        for (int k = 0; k < N; ++k) {
+            we[k] = we[k] - ac * ue[k];
+            acc += (double)we[k] * (double)we[k];
+        }
+        reinterpret_cast<V *>(w)[i] = wv;
+    }
+    if (blockIdx.x == gridDim.x - 1)
+        for (int64_t i = nvec * N + threadIdx.x; i < dim; i += blockDim.x) {
+            T q = w[i] - ac * u[i];
+            w[i] = q;
+            acc += (double)q * (double)q;
+        }
+    double s = block_sum(acc, red);
+    if (publish_and_check_last(s, partials, blockIdx.x, gridDim.x, &S->ticket, &flag)) {
+        double b2 = sum_partials(partials, gridDim.x, red);
+        if (threadIdx.x == 0) {
+            double beta = sqrt(b2), alpha = S->alpha;
+            int j = S->j;
+            alpha_out[j] = alpha;
+            beta_out[j] = beta;
+            double amax = fmax(S->amax, fabs(alpha));
+            S->amax = amax;
+            S->j = j + 1;
+            if (!isfinite(beta) || !(beta > S->tau * fmax(1.0, amax))) {
+                S->stop = 1;                      // lines 8-10
+            } else {
+                S->c_prev = S->c_cur;             // line 11, carried lazily
+                S->c_cur = 1.0 / beta;
+                S->beta = beta;
+            }
+            S->ticket = 0;
+        }
+    }
+}
+
+}  // namespace hub

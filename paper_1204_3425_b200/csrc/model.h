@@ -1,0 +1,86 @@
+// Internal model state of libhubbard_b200 (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstdint>
+#include <vector>
+
+#include "../../include/hubbard.h"
+#include "host_tables.h"
+
+namespace hub {
+
+// Hop entry encoding shared by all device tables: e = col * 2 + plus,
+// plus = 1 -> element +t, plus = 0 -> element -t.
+// Padding entries of the down ELL point at the "zero slot" col = dim_dn.
+constexpr uint32_t kPadEntry = 0xffffffffu;
+
+// Device scalars of one Lanczos run; lives in device memory, written only by
+// the finalising block of each sweep, read by every block of the next one.
+struct LanczosScalars {
+    double c_cur;    // f_j     = c_cur  * u_cur   (lazy normalisation)
+    double c_prev;   // f_{j-1} = c_prev * u_prev
+    double beta;     // b_j
+    double alpha;    // a_j of the iteration in flight
+    double amax;     // max_k |a_k| so far (breakdown rule, reading Q11)
+    double tau;
+    int j;           // iterations completed
+    int stop;        // breakdown (or bad start vector): later sweeps are no-ops
+    unsigned ticket; // arrival counter of the sweep in flight
+    unsigned pad;
+};
+
+// Everything a kernel needs to know about the model (passed by value).
+struct DevModel {
+    int64_t dim_up, dim_dn;
+    const uint32_t *st_up, *st_dn;       // basis bit patterns
+    // up table, row-major ELL [dim_up][w_up] (row-uniform access)
+    const uint32_t *up_ent;
+    const int32_t *up_cnt;
+    int w_up;
+    // down table, column-major ELL [w_dn][ld_dn] (coalesced over i_dn)
+    const uint32_t *dn_ent32;
+    const uint16_t *dn_ent16;            // compact copy when dim_dn + 1 <= 32768, else null
+    const int32_t *dn_cnt;
+    int w_dn;
+    int64_t ld_dn;
+    double t, U;
+};
+
+struct ProfRecord {
+    int kclass;
+    cudaEvent_t e0, e1;
+};
+
+}  // namespace hub
+
+struct hubbard_model {
+    int n_sites = 0, n_up = 0, n_dn = 0, dtype = HUBBARD_F64;
+    double t = 0, U = 0;
+    std::vector<int32_t> bonds;
+    hub::SpinTable up, dn;
+    bool has_device = false;
+    int variant = HUBBARD_VARIANT_AUTO;
+    double tau = -1.0;                 // < 0: default for the dtype
+    int last_cuda_error = 0;
+    int64_t launches = 0;
+    int sm_count = 148;
+    int max_smem_optin = 0;
+
+    hub::DevModel dev{};
+    std::vector<void *> dev_allocs;    // everything to cudaFree
+    // Lanczos state (allocated on first use)
+    void *work[2] = {nullptr, nullptr};
+    hub::LanczosScalars *d_scal = nullptr;
+    double *d_partial = nullptr;       // per-block partial sums
+    int64_t n_partial = 0;
+    double *d_alpha = nullptr, *d_beta = nullptr;
+    int coef_cap = 0;
+    // staging for the *_host entry points
+    void *stage[2] = {nullptr, nullptr};
+
+    bool profiling = false;
+    std::vector<hub::ProfRecord> prof;
+    int64_t prof_launches[HUBBARD_N_KCLASS] = {0};
+    double prof_ms[HUBBARD_N_KCLASS] = {0};
+};

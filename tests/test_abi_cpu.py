@@ -1,0 +1,151 @@
+"""CPU-side checks of libhubbard_b200 (no GPU, no compute calls): the library
+loads and exports every symbol include/hubbard.h declares; the host half of
+hubbard_create (basis, ranks, hop tables with signs) is bit-exact against the
+oracle on all five BASELINE configs and on small irregular sectors; argument
+validation; the host tridiagonal eigenvalue routine."""
+import ctypes
+import re
+from pathlib import Path
+
+import numpy as np
+import pytest
+
+import paper_1204_3425_b200 as hb
+from conftest import read_golden
+from inputs import CONFIGS, chain_bonds, ladder_bonds, ring_bonds, torus_bonds
+from oracle import hubbard_def as hd
+from oracle.ref import RefModel
+
+ROOT = Path(__file__).resolve().parent.parent
+
+
+def test_every_declared_symbol_is_exported():
+    header = (ROOT / "include" / "hubbard.h").read_text()
+    header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
+    declared = set(re.findall(r"\b((?:hubbard|lanczos)_\w+)\s*\(", header))
+    assert declared == set(hb.ABI_SYMBOLS), declared ^ set(hb.ABI_SYMBOLS)
+    raw = ctypes.CDLL(hb.LIB_PATH)
+    for name in declared:
+        assert hasattr(raw, name), name
+
+
+def test_paper_table1_through_the_abi():
+    """PAPER.md:67-95 (Table 1, eq. 8) via hubbard_get_basis."""
+    m = hb.hubbard_create_host(4, 2, 3, ring_bonds(4), 1.0, 0.0)
+    up, dn = m.hubbard_get_basis(0), m.hubbard_get_basis(1)
+    assert list(up) == [int(x, 2) for x in read_golden("paper_up_list.txt")[0].split()]
+    for line in read_golden("paper_table1.txt"):
+        u, d, iu, idn, J = line.split()
+        assert up[int(iu)] == int(u, 2) and dn[int(idn)] == int(d, 2)
+        assert int(iu) * m.dim_dn + int(idn) == int(J)
+    assert (m.dim_up, m.dim_dn, m.dim) == (6, 4, 24)
+
+
+def test_paper_matrix_elements_through_the_abi():
+    """PAPER.md:77-78,101-102 (eq. 9-10): signs incl. the periodic wrap, from
+    the library's own hop tables (H_hop = H_up (x) I + I (x) H_dn, eq. 14)."""
+    m = hb.hubbard_create_host(4, 2, 3, ring_bonds(4), 1.0, 0.0)
+
+    def dense(spin, n):
+        w, cols, vals = m.hubbard_get_hops(spin)
+        M = np.zeros((n, n))
+        for r in range(n):
+            for k in range(w):
+                if cols[r, k] >= 0:
+                    M[r, cols[r, k]] = vals[r, k]
+        return M
+
+    H = np.kron(dense(0, 6), np.eye(4)) + np.kron(np.eye(6), dense(1, 4))
+    for line in read_golden("paper_matrix_elements.txt"):
+        jp, j, kind, val = line.split()
+        got = H[int(jp), int(j)]
+        assert (abs(got) if kind == "abs" else got) == float(val)
+
+
+@pytest.mark.parametrize("name", ["C1", "C2", "C3", "C4", "C5"])
+def test_tables_bit_exact_vs_oracle_on_configs(name):
+    c = CONFIGS[name]
+    m = hb.hubbard_create_host(c.n_sites, c.n_up, c.n_dn, c.bonds, c.t, c.U_values[0])
+    ref = RefModel(c.n_sites, c.n_up, c.n_dn, c.bonds, c.t, c.U_values[0])
+    assert (m.dim_up, m.dim_dn, m.dim) == (c.dim_up, c.dim_dn, c.dim)
+    for spin in (0, 1):
+        assert np.array_equal(m.hubbard_get_basis(spin), ref.states[spin])
+        w, cols, vals = m.hubbard_get_hops(spin)
+        rw, rc, rv = ref.hop_ell(spin)
+        assert w == rw
+        assert np.array_equal(cols, rc)
+        assert np.array_equal(vals, rv)
+
+
+IRREGULAR = [
+    (4, 2, 3, ring_bonds(4), 1.0), (5, 2, 3, ring_bonds(5), 0.75), (6, 3, 2, ladder_bonds(2, 3) + [(0, 5)], 1.0),
+    (2, 1, 1, [(0, 1), (1, 0)], 1.0), (4, 0, 2, ring_bonds(4), 1.0), (4, 4, 2, ring_bonds(4), 1.0),
+    (7, 3, 4, ring_bonds(7) + [(0, 3), (6, 2)], 1.3), (8, 3, 5, torus_bonds(4, 2), 1.0), (4, 2, 2, chain_bonds(4), 0.0),
+    (1, 1, 0, [], 1.0),
+]
+
+
+@pytest.mark.parametrize("ns,nu,nd,bonds,t", IRREGULAR)
+def test_tables_bit_exact_vs_definition_small(ns, nu, nd, bonds, t):
+    """Against tier 0 (operator definition), including N_up != N_dn, odd rings,
+    a duplicated bond, empty and full sectors, t = 0 and a bond-free site."""
+    m = hb.hubbard_create_host(ns, nu, nd, bonds, t, 2.0)
+    sec = hd.Sector(ns, nu, nd)
+    assert list(m.hubbard_get_basis(0)) == sec.states_up and list(m.hubbard_get_basis(1)) == sec.states_dn
+    for spin in (0, 1):
+        w, cols, vals = m.hubbard_get_hops(spin)
+        rows = hd.hop_table(ns, nu, nd, spin, bonds, t)
+        assert w == max((len(r) for r in rows), default=0)
+        for r, row in enumerate(rows):
+            got = [(int(c), float(v)) for c, v in zip(cols[r], vals[r]) if c >= 0]
+            assert got == row
+            assert np.all(vals[r][cols[r] < 0] == 0.0)
+
+
+def test_create_argument_validation():
+    bad = [
+        dict(n_sites=0, n_up=0, n_dn=0, bonds=[]), dict(n_sites=33, n_up=1, n_dn=1, bonds=[(0, 1)]),
+        dict(n_sites=4, n_up=5, n_dn=1, bonds=ring_bonds(4)), dict(n_sites=4, n_up=-1, n_dn=1, bonds=ring_bonds(4)),
+        dict(n_sites=4, n_up=2, n_dn=2, bonds=[(0, 4)]), dict(n_sites=4, n_up=2, n_dn=2, bonds=[(1, 1)]),
+        dict(n_sites=4, n_up=2, n_dn=2, bonds=[(-1, 2)]),
+    ]
+    for kw in bad:
+        with pytest.raises(hb.HubbardError) as ei:
+            hb.hubbard_create_host(t=1.0, U=1.0, **kw)
+        assert ei.value.code == -1
+    with pytest.raises(hb.HubbardError) as ei:
+        hb.hubbard_create_host(4, 2, 2, ring_bonds(4), float("nan"), 1.0)
+    assert ei.value.code == -1
+    with pytest.raises(hb.HubbardError) as ei:       # C(32,16) = 601080390 fits, C(32,16)... use a sector >= 2^31-1: none at N_s<=32
+        hb.hubbard_create_host(4, 2, 2, ring_bonds(4), 1.0, float("inf"))
+    assert ei.value.code == -1
+
+
+def test_host_only_model_refuses_compute():
+    m = hb.hubbard_create_host(4, 2, 2, ring_bonds(4), 1.0, 4.0)
+    x = np.zeros(m.dim)
+    rc = hb.lib.hubbard_apply(m._h, x.ctypes.data, x.ctypes.data, None)
+    assert rc == -5
+    a = np.zeros(4)
+    dp = ctypes.POINTER(ctypes.c_double)
+    rc = hb.lib.lanczos_run(m._h, x.ctypes.data, 4, a.ctypes.data_as(dp), a.ctypes.data_as(dp), None, None)
+    assert rc == -5
+    assert b"no device" in hb.lib.hubbard_strerror(-5)
+    m.hubbard_destroy()
+    m.hubbard_destroy()  # idempotent
+    hb.lib.hubbard_destroy(None)
+
+
+def test_ground_energy_vs_lapack():
+    rng = np.random.default_rng(7)
+    for m in (1, 2, 3, 17, 200):
+        a = rng.normal(size=m) * 3
+        b = np.abs(rng.normal(size=max(m - 1, 1))) + 0.1
+        T = np.diag(a) + np.diag(b[:m - 1], 1) + np.diag(b[:m - 1], -1)
+        e = hb.lanczos_ground_energy(a, b, m)
+        assert abs(e - np.linalg.eigvalsh(T)[0]) <= 1e-13 * max(1.0, np.abs(T).sum(axis=1).max())
+    # zero off-diagonals (breakdown leaves beta ~ 0), prefix m < len
+    assert hb.lanczos_ground_energy([3.0, -1.0, 2.0], [0.0, 0.0]) == pytest.approx(-1.0, abs=1e-14)
+    assert hb.lanczos_ground_energy([3.0, -1.0, 2.0], [0.0, 0.0], 1) == pytest.approx(3.0, abs=1e-14)
+    with pytest.raises(hb.HubbardError):
+        hb.lanczos_ground_energy([float("nan")], [0.0], 1)
