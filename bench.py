@@ -1,0 +1,363 @@
+#!/usr/bin/env python
+"""bench.py — the headline measurement (BASELINE.json `metric`): H*v/s and HBM
+GB/s as a fraction of the measured peak for the fused Lanczos H*v on the 4x4
+half-filled Hubbard lattice (config C4), through the C ABI.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C4] [--dtype f64|f32|both]
+    python bench.py --impl reference ...      # the CPU oracle as it stands, on the host cores
+
+A "step" is one whole Lanczos job of the config (`iters` iterations of
+Algorithm 1: fused H*v + vector updates) on a
+seeded synthetic start vector.  `value` = Lanczos iterations (= fused H*v) per
+second over all ranks.  Multi-GPU = independent replicas:
+no data-path collective, weak scaling.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+from pathlib import Path
+
+ROOT = Path(__file__).resolve().parent
+if str(ROOT) not in sys.path:
+    sys.path.insert(0, str(ROOT))
+
+METRIC = "fused Lanczos H*v per second (Lanczos iterations/s), 4x4 half-filled Hubbard"
+UNIT = "Hv/s"
+FALLBACK_HBM_GBS = 6650.0      # /opt/skills/guides/B200_PROFILING.md fallback
+
+
+def parse_args():
+    p = argparse.ArgumentParser()
+    p.add_argument("--gpus", type=int, default=1)
+    p.add_argument("--steps", type=int, default=3)
+    p.add_argument("--warmup", type=int, default=3)
+    p.add_argument("--impl", default="native", choices=["native", "reference"])
+    p.add_argument("--config", default="C4")
+    p.add_argument("--dtype", default="both", choices=["f64", "f32", "both"])
+    p.add_argument("--U", type=float, default=None)
+    p.add_argument("--iters", type=int, default=None, help="Lanczos iterations per step (default: the config's)")
+    p.add_argument("--variant", default="auto", choices=["auto", "paper", "twosweep"])
+    p.add_argument("--no-cpu-baseline", action="store_true")
+    p.add_argument("--no-e2e", action="store_true")
+    return p.parse_args()
+
+
+def hbm_peak():
+    f = ROOT / "MEASURED_PEAKS.json"
+    if f.exists():
+        try:
+            return float(json.loads(f.read_text())["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.path = index, None, None
+
+    def start(self):
+        try:
+            fd, self.path = tempfile.mkstemp(suffix=".csv")
+            os.close(fd)
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if not self.proc:
+            return out
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, smax, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in Path(self.path).read_text().splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); smax.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        os.unlink(self.path)
+        if sm:
+            sm.sort()
+            out.update(sm_mhz=sm[len(sm) // 2], sm_max_mhz=max(smax), power_w_max=max(pw), reasons=sorted(reasons),
+                       samples=len(sm))
+        return out
+
+
+def dist_setup(n_gpus: int):
+    import torch
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        backend = "nccl" if torch.cuda.is_available() else "gloo"
+        if torch.cuda.is_available():
+            torch.cuda.set_device(local)
+        dist.init_process_group(backend=backend)
+    return rank, world, local
+
+
+def barrier(world):
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+
+
+def max_over_ranks(x: float, world: int, device) -> float:
+    if world == 1:
+        return x
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+# --------------------------------------------------------------------- CPU leg
+def cpu_oracle_prepare(cfg, U):
+    import numpy as np
+    from inputs import start_vector_np
+    from oracle import ref as oref
+
+    m = oref.RefModel(cfg.n_sites, cfg.n_up, cfg.n_dn, cfg.bonds, cfg.t, U)
+    v0 = start_vector_np(cfg.seed, cfg.dim)
+    v0 /= np.sqrt(np.dot(v0, v0))
+    return m, v0
+
+
+def cpu_oracle_sample(cfg, prepared, iters_sample, n_threads=0):
+    """The oracle as it stands (tier 1: oracle/hubbard_ref.c, the paper's CPU
+    comparator restated) timed on the host cores: `iters_sample` Lanczos
+    iterations of Algorithm 1 + eq. 13 on the full vector of the workload."""
+    from oracle import ref as oref
+
+    m, v0 = prepared
+    cores = oref.max_threads() if n_threads == 0 else n_threads
+    t0 = time.perf_counter()
+    a, b = m.lanczos_two_vector(v0, iters_sample, n_threads=n_threads)
+    dt = time.perf_counter() - t0
+    return {"value": len(a) / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"{len(a)} Lanczos iterations (Algorithm 1 + eq. 13, fp64, CSR hops) on the full "
+                      f"{cfg.name} vector (dim {cfg.dim}), {dt:.1f} s"}, dt
+
+
+def sample_iters_for(cfg):
+    # ~10-30 s of CPU work: an H*v on C4 costs a few seconds on a many-core host
+    if cfg.dim > 5e8:
+        return 1
+    if cfg.dim > 5e7:
+        return 3
+    if cfg.dim > 5e6:
+        return 20
+    return cfg.iters
+
+
+def run_reference(args):
+    from inputs import CONFIGS
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    cfg = CONFIGS[args.config]
+    U = args.U if args.U is not None else cfg.U_values[-1]
+    n = sample_iters_for(cfg)
+    total_iters, total_t, last = 0, 0.0, None
+    prepared = cpu_oracle_prepare(cfg, U)
+    if args.warmup > 0:
+        cpu_oracle_sample(cfg, prepared, 1)
+    for _ in range(args.steps):
+        last, dt = cpu_oracle_sample(cfg, prepared, n)
+        total_iters += n
+        total_t += dt
+    val = total_iters / total_t
+    last["value"] = val
+    line = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total_t / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"{cfg.name} {cfg.lattice} {cfg.n_up}up{cfg.n_dn}dn dim={cfg.dim} U={U}",
+                   "step": f"bounded sample: {n} Lanczos iterations of the CPU oracle per step"},
+        "cpu_baseline": last,
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+# --------------------------------------------------------------------- GPU leg
+def run_native_dtype(args, cfg, U, dtype, rank, world, local):
+    import numpy as np
+    import torch
+
+    import paper_1204_3425_b200 as hb
+    from inputs import start_vector_torch
+
+    dev = torch.device("cuda", local)
+    tdt = torch.float64 if dtype == "f64" else torch.float32
+    s = 8 if dtype == "f64" else 4
+    iters = args.iters or cfg.iters
+    variant = {"auto": hb.VARIANT_AUTO, "paper": hb.VARIANT_PAPER, "twosweep": hb.VARIANT_TWOSWEEP}[args.variant]
+
+    m = hb.hubbard_create(cfg.n_sites, cfg.n_up, cfg.n_dn, cfg.bonds, cfg.t, U, dtype)
+    m.hubbard_set_variant(variant)
+    v0 = start_vector_torch(cfg.seed + rank, cfg.dim, dev, torch.float64)
+    v0 /= torch.linalg.vector_norm(v0)
+    v0 = v0.to(tdt).contiguous()
+    stream = torch.cuda.current_stream()
+
+    for _ in range(args.warmup):
+        alpha, beta = m.lanczos_run(v0, iters, stream)
+    torch.cuda.synchronize()
+    barrier(world)
+
+    # ---- timed region: K whole Lanczos jobs, inputs resident in HBM
+    clocks = ClockSampler(local)
+    clocks.start()
+    m.hubbard_profile(True)
+    l0 = m.hubbard_launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record(stream)
+    done = 0
+    for _ in range(args.steps):
+        alpha, beta = m.lanczos_run(v0, iters, stream)
+        done += len(alpha)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    barrier(world)
+    ms = max_over_ranks(e0.elapsed_time(e1), world, dev)
+    launches = m.hubbard_launch_count() - l0
+    ktimes = m.hubbard_kernel_times()
+    m.hubbard_profile(False)
+    clk = clocks.stop()
+    assert done == args.steps * iters, f"Lanczos stopped early ({done} of {args.steps * iters} iterations)"
+    e_0 = hb.lanczos_ground_energy(alpha, beta)
+
+    # ---- per-kernel device times (CUDA events on the launching stream, inside the timed region)
+    peak, peak_src = hbm_peak()
+    kern = {}
+    for name, (n, tms) in ktimes.items():
+        if n:
+            kern[name] = {"launches": n, "avg_ms": tms / n}
+    hv_ms = sum(kern[k]["avg_ms"] for k in ("hv_paper", "row_sweep", "strip_sweep") if k in kern)
+    hv_parts = "+".join(k for k in ("hv_paper", "row_sweep", "strip_sweep") if k in kern)
+    hv_bytes = 3 * cfg.dim * s                       # read f_j, read f_{j-1}, write q_j
+    iter_ms = ms / (args.steps * iters)
+    roof = {
+        "bound": "hbm", "kernel": f"fused Lanczos H*v ({hv_parts})",
+        "achieved": hv_bytes / (hv_ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
+        "traffic": None, "algorithmic_bytes_per_launch": hv_bytes, "avg_ms": hv_ms, "peak_source": peak_src,
+        "whole_iteration": {"algorithmic_bytes": 6 * cfg.dim * s, "ms": iter_ms,
+                            "achieved": 6 * cfg.dim * s / (iter_ms * 1e-3) / 1e9},
+    }
+    roof["frac"] = roof["achieved"] / peak
+    roof["whole_iteration"]["frac"] = roof["whole_iteration"]["achieved"] / peak
+    for k, d in kern.items():
+        if k in ("row_sweep", "strip_sweep", "hv_paper", "axpy_norm"):
+            d["algorithmic_bytes"] = 3 * cfg.dim * s
+            d["GBps"] = d["algorithmic_bytes"] / (d["avg_ms"] * 1e-3) / 1e9
+
+    # ---- end to end: host start vector (pinned) -> lanczos_run_host -> alpha/beta on the host
+    e2e = None
+    if not args.no_e2e:
+        vh = torch.empty(cfg.dim, dtype=tdt, pin_memory=True)
+        vh.copy_(v0)
+        m.lanczos_run_host(vh, min(iters, 5), stream)
+        torch.cuda.synchronize()
+        barrier(world)
+        t0 = time.perf_counter()
+        n_e2e = 0
+        for _ in range(args.steps):
+            a, b = m.lanczos_run_host(vh, iters, stream)      # synchronises; alpha/beta land on the host
+            n_e2e += len(a)
+        torch.cuda.synchronize()
+        dt = max_over_ranks(time.perf_counter() - t0, world, dev)
+        e2e = {"value": world * n_e2e / dt, "unit": UNIT, "h2d_bytes_per_step": cfg.dim * s,
+               "d2h_bytes_per_step": 2 * iters * 8, "ms_per_step": 1e3 * dt / args.steps}
+    del v0
+    m.close()
+    torch.cuda.empty_cache()
+    return {
+        "dtype": dtype, "value": world * args.steps * iters / (ms * 1e-3), "ms_per_step": ms / args.steps,
+        "s_per_iteration": iter_ms * 1e-3, "roofline": roof, "kernels": kern, "e2e": e2e,
+        "gpu_launches": launches, "clocks": clk, "E0": e_0, "iters": iters,
+    }
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    import torch
+    from inputs import CONFIGS
+
+    if not torch.cuda.is_available():
+        print("bench.py: no CUDA device; the hot path has no CPU fallback", file=sys.stderr)
+        return 2
+    rank, world, local = dist_setup(args.gpus)
+    torch.cuda.set_device(local)
+    cfg = CONFIGS[args.config]
+    U = args.U if args.U is not None else cfg.U_values[-1]
+    dtypes = ["f64", "f32"] if args.dtype == "both" else [args.dtype]
+    dtypes = [d for d in dtypes if d in cfg.dtypes] or dtypes[:1]
+    results = {d: run_native_dtype(args, cfg, U, d, rank, world, local) for d in dtypes}
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cpu, _ = cpu_oracle_sample(cfg, cpu_oracle_prepare(cfg, U), sample_iters_for(cfg))
+    if rank == 0:
+        main_r = results[dtypes[0]]
+        line = {
+            "metric": METRIC, "value": main_r["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": main_r["ms_per_step"], "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": main_r["dtype"], "data": "synthetic",
+            "config": {"workload": f"{cfg.name} {cfg.lattice} {cfg.n_up}up{cfg.n_dn}dn dim={cfg.dim} t={cfg.t} U={U}",
+                       "step": f"one Lanczos job of {main_r['iters']} iterations (fused H*v + vector updates)",
+                       "start_vector": f"seeded uniform[-1,1) normalised, seed {cfg.seed}+rank",
+                       "l2": "inputs exceed L2 (no flush needed)" if cfg.dim * 4 > 2 * 126e6 else
+                             "inputs fit in L2: cache-resident by design (DESIGN.md), HBM fraction not meaningful",
+                       "variant": args.variant, "parallelism": "replicas" if world > 1 else "single GPU"},
+            "s_per_iteration": main_r["s_per_iteration"],
+            "roofline": main_r["roofline"], "kernels": main_r["kernels"], "e2e": main_r["e2e"],
+            "gpu_launches": main_r["gpu_launches"], "clocks": main_r["clocks"], "E0": main_r["E0"],
+        }
+        if cpu is not None:
+            line["cpu_baseline"] = cpu
+        for d in dtypes[1:]:
+            r = results[d]
+            line[d] = {k: r[k] for k in ("value", "ms_per_step", "s_per_iteration", "roofline", "kernels", "e2e",
+                                         "gpu_launches", "clocks", "E0")}
+        print(json.dumps(line))
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

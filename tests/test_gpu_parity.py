@@ -1,0 +1,315 @@
+"""GPU parity tests (run on the B200 box with `-m gpu`): the CUDA path, called
+through the C ABI (paper_1204_3425_b200.binding -> libhubbard_b200.so), against
+the CPU oracle element by element on the same seeded inputs.
+
+Tolerances are BASELINE.json's: H*v relative max-norm error <= 1e-12 (fp64) /
+1e-5 (fp32); E_0 after a fixed iteration count <= 1e-10 / 1e-5 relative;
+alpha_j, beta_j compared on the prefix of DESIGN.md reading Q12.
+"""
+import numpy as np
+import pytest
+import torch
+
+import paper_1204_3425_b200 as hb
+from inputs import CONFIGS, chain_bonds, g_uniform, ladder_bonds, ring_bonds, sample_indices, start_vector_torch, torus_bonds
+from oracle import hubbard_def as hd
+from oracle import lanczos_ref as lr
+from oracle.ref import RefModel
+
+pytestmark = pytest.mark.gpu
+
+TOL_HV = {"f64": 1e-12, "f32": 1e-5}
+TOL_E0 = {"f64": 1e-10, "f32": 1e-5}
+TDT = {"f64": torch.float64, "f32": torch.float32}
+VARIANTS = {"paper": hb.VARIANT_PAPER, "twosweep": hb.VARIANT_TWOSWEEP, "auto": hb.VARIANT_AUTO}
+
+
+def dev():
+    assert torch.cuda.is_available(), "these tests need the B200 (no CPU fallback exists)"
+    return torch.device("cuda:0")
+
+
+def start_vector(seed, dim, dtype):
+    """Seeded uniform[-1,1) vector, normalised in fp64, rounded to `dtype`
+    (reading Q13).  Returns (device tensor, the same bits as fp64 numpy)."""
+    v = start_vector_torch(seed, dim, dev(), torch.float64)
+    v /= torch.linalg.vector_norm(v)
+    v = v.to(TDT[dtype]).contiguous()
+    return v, v.double().cpu().numpy()
+
+
+def rel_max_err(y_gpu, y_ref):
+    y = y_gpu.double().cpu().numpy()
+    return float(np.max(np.abs(y - y_ref)) / max(np.max(np.abs(y_ref)), 1e-300))
+
+
+SMALL = [
+    (2, 1, 1, [(0, 1)]),
+    (4, 2, 3, ring_bonds(4)),
+    (5, 2, 3, ring_bonds(5)),
+    (6, 3, 3, ring_bonds(6)),
+    (6, 2, 4, ladder_bonds(3, 2)),
+    (6, 1, 5, chain_bonds(6)),
+    (7, 3, 4, ring_bonds(7) + [(0, 3), (2, 6)]),
+    (6, 0, 3, ring_bonds(6)),
+    (6, 3, 6, ring_bonds(6)),
+    (5, 0, 0, ring_bonds(5)),
+    (5, 5, 5, ring_bonds(5)),
+]
+
+
+@pytest.mark.parametrize("variant", ["paper", "twosweep"])
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("ns,nu,nd,bonds", SMALL)
+def test_apply_vs_definition_small(ns, nu, nd, bonds, dtype, variant):
+    """H*v against the dense H built from the operator definition (tier 0),
+    including N_up != N_dn, odd rings, non-ring bond lists, and the degenerate
+    sectors dim_up = 1, dim_dn = 1, dim = 1."""
+    t, U = 0.75, 3.5
+    H = hd.dense_hamiltonian(ns, nu, nd, bonds, t, U)
+    m = hb.hubbard_create(ns, nu, nd, bonds, t, U, dtype)
+    m.hubbard_set_variant(VARIANTS[variant])
+    assert m.dim == H.shape[0]
+    x, x_np = start_vector(77 + ns, m.dim, dtype)
+    y = torch.full_like(x, float("nan"))
+    m.hubbard_apply(x, y)
+    torch.cuda.synchronize()
+    y_ref = H @ x_np
+    if np.max(np.abs(y_ref)) == 0.0:
+        assert float(y.abs().max()) == 0.0
+    else:
+        assert rel_max_err(y, y_ref) <= TOL_HV[dtype]
+
+
+@pytest.mark.parametrize("variant", ["paper", "twosweep"])
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("name", ["C1", "C2", "C3"])
+def test_apply_full_vector_C1_C2_C3(name, dtype, variant):
+    c = CONFIGS[name]
+    for U in c.U_values:
+        ref = RefModel(c.n_sites, c.n_up, c.n_dn, c.bonds, c.t, U)
+        m = hb.hubbard_create(c.n_sites, c.n_up, c.n_dn, c.bonds, c.t, U, dtype)
+        m.hubbard_set_variant(VARIANTS[variant])
+        x, x_np = start_vector(c.seed, c.dim, dtype)
+        y = torch.full_like(x, float("nan"))
+        m.hubbard_apply(x, y)
+        torch.cuda.synchronize()
+        assert rel_max_err(y, ref.apply(x_np)) <= TOL_HV[dtype]
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_apply_full_vector_C4(dtype):
+    """Headline config at full size, in the launch configuration bench.py
+    times (variant AUTO), against the tier-1 oracle over the whole vector."""
+    c = CONFIGS["C4"]
+    U = 8.0
+    ref = RefModel(c.n_sites, c.n_up, c.n_dn, c.bonds, c.t, U)
+    m = hb.hubbard_create(c.n_sites, c.n_up, c.n_dn, c.bonds, c.t, U, dtype)
+    x, x_np = start_vector(c.seed, c.dim, dtype)
+    y = torch.full_like(x, float("nan"))
+    m.hubbard_apply(x, y)
+    torch.cuda.synchronize()
+    y_ref = ref.apply(x_np)
+    assert rel_max_err(y, y_ref) <= TOL_HV[dtype]
+    # the comparator kernel on the same input
+    m.hubbard_set_variant(hb.VARIANT_PAPER)
+    y.fill_(float("nan"))
+    m.hubbard_apply(x, y)
+    torch.cuda.synchronize()
+    assert rel_max_err(y, y_ref) <= TOL_HV[dtype]
+
+
+def _sampled_parity(name, dtype, n_samples, U):
+    """Pin P10: (H v0)[J] on seeded sample indices from the operator
+    definition (tier 0), v0[J] = g(seed, J) un-normalised."""
+    c = CONFIGS[name]
+    m = hb.hubbard_create(c.n_sites, c.n_up, c.n_dn, c.bonds, c.t, U, dtype)
+    x = start_vector_torch(c.seed, c.dim, dev(), TDT[dtype])
+    y = torch.empty_like(x)
+    m.hubbard_apply(x, y)
+    torch.cuda.synchronize()
+    J = sample_indices(c.seed + 1000, c.dim, n_samples)
+    sec = hd.Sector(c.n_sites, c.n_up, c.n_dn)
+
+    def v_of(idx):
+        v = g_uniform(c.seed, idx)
+        return v.astype(np.float32).astype(np.float64) if dtype == "f32" else v
+
+    y_ref = hd.sampled_Hv(sec, c.bonds, c.t, U, J, v_of)
+    y_s = y[torch.from_numpy(J).to(dev())].double().cpu().numpy()
+    scale = float(y.abs().max())
+    assert np.max(np.abs(y_s - y_ref)) / scale <= TOL_HV[dtype]
+    return m, x, y
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_apply_sampled_vs_definition_C4(dtype):
+    _sampled_parity("C4", dtype, 600, 4.0)
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_apply_sampled_vs_definition_C5(dtype):
+    """dim = 2 363 904 400 > 2^31: 64-bit offsets; V row larger than one SM's
+    shared memory in fp64."""
+    free, _ = torch.cuda.mem_get_info()
+    need = 2 * CONFIGS["C5"].dim * (8 if dtype == "f64" else 4) + (4 << 30)
+    if free < need:
+        pytest.skip(f"needs {need >> 30} GiB of free HBM")
+    _sampled_parity("C5", dtype, 300, 4.0)
+    torch.cuda.empty_cache()
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_full_scale_invariants_C4(dtype):
+    """Pin P9 at full scale, oracle-free: Hermiticity, U-linearity of the
+    diagonal with its closed form, spin-swap H(V^T) = (H V)^T."""
+    c = CONFIGS["C4"]
+    tol = 1e-11 if dtype == "f64" else 2e-5
+    m = hb.hubbard_create(c.n_sites, c.n_up, c.n_dn, c.bonds, c.t, 8.0, dtype)
+    x, _ = start_vector(c.seed, c.dim, dtype)
+    z, _ = start_vector(c.seed + 7, c.dim, dtype)
+    hx, hz = torch.empty_like(x), torch.empty_like(x)
+    m.hubbard_apply(x, hx)
+    m.hubbard_apply(z, hz)
+    a = torch.dot(z.double(), hx.double()).item()
+    b = torch.dot(hz.double(), x.double()).item()
+    scale = torch.linalg.vector_norm(hx.double()).item() * torch.linalg.vector_norm(z.double()).item()
+    assert abs(a - b) / scale <= tol
+    # (ii) H(U) x - H(0) x = U popcount(up & dn) o x
+    m.hubbard_set_U(0.0)
+    h0 = torch.empty_like(x)
+    m.hubbard_apply(x, h0)
+    st_up = torch.from_numpy(m.hubbard_get_basis(0).astype(np.int64)).to(dev())
+    st_dn = torch.from_numpy(m.hubbard_get_basis(1).astype(np.int64)).to(dev())
+    diff = (hx.double() - h0.double()).view(m.dim_up, m.dim_dn)
+    ymax = hx.abs().max().item()
+    worst = 0.0
+    for r0 in range(0, m.dim_up, 1024):
+        r1 = min(m.dim_up, r0 + 1024)
+        both = st_up[r0:r1, None] & st_dn[None, :]
+        docc = torch.zeros_like(both)
+        for k in range(c.n_sites):
+            docc += (both >> k) & 1
+        want = 8.0 * docc.double() * x.view(m.dim_up, m.dim_dn)[r0:r1].double()
+        worst = max(worst, (diff[r0:r1] - want).abs().max().item())
+    assert worst / ymax <= tol
+    # (iii) spin swap (N_up = N_dn, one bond list)
+    m.hubbard_set_U(8.0)
+    xt = x.view(m.dim_up, m.dim_dn).t().contiguous().view(-1)
+    hxt = torch.empty_like(x)
+    m.hubbard_apply(xt, hxt)
+    err = (hxt.view(m.dim_dn, m.dim_up).t() - hx.view(m.dim_up, m.dim_dn)).abs().max().item()
+    assert err / ymax <= tol
+
+
+def _lanczos_case(name, U, dtype, variant, iters, n_prefix):
+    c = CONFIGS[name]
+    ref = RefModel(c.n_sites, c.n_up, c.n_dn, c.bonds, c.t, U)
+    m = hb.hubbard_create(c.n_sites, c.n_up, c.n_dn, c.bonds, c.t, U, dtype)
+    m.hubbard_set_variant(VARIANTS[variant])
+    v0, v0_np = start_vector(c.seed, c.dim, dtype)
+    keep = v0.clone()
+    alpha, beta = m.lanczos_run(v0, iters)
+    assert torch.equal(v0, keep), "lanczos_run must not modify v0"
+    a_ref, b_ref = lr.lanczos(ref.apply, v0_np, iters)
+    assert len(alpha) == len(a_ref) == iters
+    tol_c = 1e-10 if dtype == "f64" else 1e-5
+    n = min(n_prefix, iters)
+    assert np.max(np.abs(alpha[:n] - a_ref[:n]) / np.maximum(1.0, np.abs(a_ref[:n]))) <= tol_c
+    assert np.max(np.abs(beta[:n] - b_ref[:n]) / np.maximum(1.0, np.abs(b_ref[:n]))) <= tol_c
+    e_gpu = hb.lanczos_ground_energy(alpha, beta)
+    e_ref = lr.ground_energy(a_ref, b_ref)
+    assert abs(e_gpu - e_ref) / abs(e_ref) <= TOL_E0[dtype]
+    return e_gpu
+
+
+@pytest.mark.parametrize("variant", ["paper", "twosweep"])
+def test_lanczos_C1(variant):
+    e = _lanczos_case("C1", 4.0, "f64", variant, 100, 50)
+    assert abs(e - (-4.603526299989)) < 1e-9          # SURVEY P11, also dense eigvalsh in the CPU suite
+
+
+@pytest.mark.parametrize("variant", ["paper", "twosweep"])
+@pytest.mark.parametrize("dtype,n_prefix", [("f64", 50), ("f32", 30)])
+@pytest.mark.parametrize("U", [4.0, 8.0])
+def test_lanczos_C2(U, dtype, n_prefix, variant):
+    _lanczos_case("C2", U, dtype, variant, 200, n_prefix)
+
+
+@pytest.mark.parametrize("dtype,n_prefix", [("f64", 40), ("f32", 30)])
+def test_lanczos_C3_prefix(dtype, n_prefix):
+    """C3 with a shortened run (the oracle's H*v costs ~0.3 s here): prefix of
+    alpha/beta and E_0^(m) at m = 40."""
+    _lanczos_case("C3", 8.0, dtype, "auto", 40, n_prefix)
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_lanczos_C4_free_fermions(dtype):
+    """Pin P6 at full scale, oracle-free: U = 0 on the 4x4 half-filled torus,
+    E_0 = -24 (two copies of the lowest 8 levels of -2(cos kx + cos ky)).
+    Wrong wrap signs would give hard-core-boson energies instead."""
+    c = CONFIGS["C4"]
+    m = hb.hubbard_create(c.n_sites, c.n_up, c.n_dn, c.bonds, c.t, 0.0, dtype)
+    v0, _ = start_vector(c.seed, c.dim, dtype)
+    alpha, beta = m.lanczos_run(v0, 200)
+    assert len(alpha) == 200
+    e = hb.lanczos_ground_energy(alpha, beta)
+    tol = 1e-7 if dtype == "f64" else 2e-5
+    assert -24.0 - 24.0 * tol <= e <= -24.0 + 24.0 * (2e-5 if dtype == "f32" else 1e-6)
+
+
+def test_lanczos_breakdown_atomic_limit():
+    """t = 0: H is diagonal with few distinct values; the Krylov space is
+    exhausted and lanczos_run stops early (Algorithm 1 lines 8-10, reading
+    Q11) exactly where the oracle does."""
+    ns, nu, nd, bonds = 6, 3, 3, ring_bonds(6)
+    ref = RefModel(ns, nu, nd, bonds, 0.0, 4.0)
+    for variant in ("paper", "twosweep"):
+        m = hb.hubbard_create(ns, nu, nd, bonds, 0.0, 4.0, "f64")
+        m.hubbard_set_variant(VARIANTS[variant])
+        v0, v0_np = start_vector(5, m.dim, "f64")
+        alpha, beta = m.lanczos_run(v0, 50)
+        a_ref, b_ref = lr.lanczos(ref.apply, v0_np, 50)
+        assert len(alpha) == len(a_ref) < 50
+        assert abs(hb.lanczos_ground_energy(alpha, beta) - 0.0) < 1e-9     # U * max(0, N - N_s) = 0
+
+
+def test_edge_cases_and_errors():
+    m = hb.hubbard_create(6, 3, 3, ring_bonds(6), 1.0, 4.0, "f64")
+    x, _ = start_vector(1, m.dim, "f64")
+    with pytest.raises(hb.HubbardError):
+        m.hubbard_apply(x, x)                               # aliasing
+    a, b = m.lanczos_run(x, 0)
+    assert len(a) == 0 and len(b) == 0
+    # zero start vector: no iteration can be done
+    a, b = m.lanczos_run(torch.zeros_like(x), 5)
+    assert len(a) == 0
+    # host-buffer entry points give the same bits as the device ones
+    y = torch.empty_like(x)
+    m.hubbard_apply(x, y)
+    torch.cuda.synchronize()
+    yh = np.empty(m.dim)
+    m.hubbard_apply_host(x.cpu().numpy(), yh)
+    assert np.array_equal(yh, y.cpu().numpy())
+    a1, b1 = m.lanczos_run(x, 20)
+    a2, b2 = m.lanczos_run_host(x.cpu().numpy(), 20)
+    assert np.array_equal(a1, a2) and np.array_equal(b1, b2)
+    # run-to-run determinism of the reductions
+    a3, b3 = m.lanczos_run(x, 20)
+    assert np.array_equal(a1, a3) and np.array_equal(b1, b3)
+    assert m.hubbard_launch_count() > 0
+
+
+def test_non_default_stream():
+    c = CONFIGS["C2"]
+    m = hb.hubbard_create(c.n_sites, c.n_up, c.n_dn, c.bonds, c.t, 4.0, "f64")
+    x, _ = start_vector(c.seed, c.dim, "f64")
+    y0, y1 = torch.empty_like(x), torch.empty_like(x)
+    m.hubbard_apply(x, y0)
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        m.hubbard_apply(x, y1)
+    s.synchronize()
+    torch.cuda.synchronize()
+    assert torch.equal(y0, y1)
