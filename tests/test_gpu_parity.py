@@ -247,15 +247,21 @@ def test_lanczos_C3_prefix(dtype, n_prefix):
 def test_lanczos_C4_free_fermions(dtype):
     """Pin P6 at full scale, oracle-free: U = 0 on the 4x4 half-filled torus,
     E_0 = -24 (two copies of the lowest 8 levels of -2(cos kx + cos ky)).
-    Wrong wrap signs would give hard-core-boson energies instead."""
+    Wrong wrap signs would give hard-core-boson energies instead.  The
+    single-particle levels are -4, -2, 0, 2, 4, so H has only the 25 distinct
+    eigenvalues -24, -22, ..., 24: the Krylov space is exhausted after 25
+    steps and lanczos_run must stop there (Algorithm 1 lines 8-10, reading Q11)."""
     c = CONFIGS["C4"]
     m = hb.hubbard_create(c.n_sites, c.n_up, c.n_dn, c.bonds, c.t, 0.0, dtype)
     v0, _ = start_vector(c.seed, c.dim, dtype)
     alpha, beta = m.lanczos_run(v0, 200)
-    assert len(alpha) == 200
+    if dtype == "f64":
+        assert len(alpha) == 25
+    else:
+        assert 25 <= len(alpha) <= 200
     e = hb.lanczos_ground_energy(alpha, beta)
-    tol = 1e-7 if dtype == "f64" else 2e-5
-    assert -24.0 - 24.0 * tol <= e <= -24.0 + 24.0 * (2e-5 if dtype == "f32" else 1e-6)
+    tol = 1e-10 if dtype == "f64" else 1e-5
+    assert abs(e + 24.0) <= 24.0 * tol
 
 
 def test_lanczos_breakdown_atomic_limit():
