@@ -1,0 +1,320 @@
+// Variant GATHER: H v as two symmetric "gather sweeps".
+//
+// H_hop is a Kronecker SUM (eq. 14): the down term couples
+// elements of one ROW of V, the up term elements of one COLUMN.  Both sweeps
+// therefore use the same device code on a tile that is closed under its term:
+//
+//   ROW sweep  tile = R whole rows    (a0..a0+R-1, all b)   contracts H_dn   eq. 16 + Algorithm 4
+//   COL sweep  tile = R whole columns (all a, c0..c0+R-1)   contracts H_up   eq. 15
+//
+// The tile is staged in shared memory INTERLEAVED, Xs[i][r] (i = the contracted
+// index, r = 0..R-1 the tile's rows/columns), R*sizeof(T) = 16 bytes when it
+// fits, so that ONE 128-bit shared-memory load fetches the hop source of all R
+// outputs a thread owns; the hop entry (Algorithms 2/3: Aj, Ax of the ELL
+// format, column-major so that a warp reads them coalesced)
+// is read once per R outputs.  Padding entries point at a zero slot.
+//
+// Lanczos form (Algorithm 1 with eq. 13), 8 vector passes per
+// iteration, no separate axpy/norm kernel:
+//   ROW sweep of iteration j+1:  w = q_j - a_j f_j  (line 6; staged AND written
+//        over q_j), b_{j+1}^2 = |w|^2 (line 7), z = (t H_dn + D) w  -> buffer Z;
+//        the last block records a_j, b_{j+1}, applies lines 8-10 and carries
+//        f_{j+1} = w / b_{j+1} (line 11) as the scalar c = 1/b_{j+1}.
+//   COL sweep of iteration j+1:  q_{j+1} = c (t H_up w + z) - b_{j+1} f_j  (line 4,
+//        written over f_j as in eq. 13) and a_{j+1} = q_{j+1} . f_{j+1} (line 5).
+#pragma once
+#include "kernels_common.cuh"
+
+namespace hub {
+
+constexpr int kGatherThreads = 1024;
+constexpr int kGatherBatch = 8;          // hop entries fetched ahead per thread
+
+// One spin's hop table in the device layout of this variant: column-major ELL
+// [w][ld], entry = col * 2 + neg, the matrix element being t * (neg ? -1 : +1)
+// (PAPER.md:99-104); padding entries are dim * 2 (the zero slot, sign +).
+struct SpinDev {
+    int64_t dim;            // dim_sigma
+    int64_t ld;             // leading dimension of the ELL arrays (multiple of 32)
+    int w;                  // ELL width
+    const uint16_t *e16;    // entries when dim + 1 <= 32768, else null
+    const uint32_t *e32;    // entries (always present)
+    const int32_t *cnt;     // hops per state
+    const uint32_t *st;     // basis bit patterns
+};
+
+template <typename T>
+struct GatherArgs {
+    SpinDev in;             // the spin whose index is contracted (dn for ROW, up for COL)
+    const uint32_t *st_out; // bit patterns of the other spin (ROW: states_up, for the diagonal)
+    int64_t dim_up, dim_dn;
+    double t, U;
+    // plain apply: y = H x
+    const T *x;
+    T *y;
+    // Lanczos: Q holds q_j -> w, F holds u_j (f_j = c_j u_j) -> q_{j+1}, Z the row-sweep result
+    T *Q, *F, *Z;
+    LanczosScalars *S;
+    double *partials;
+    double *alpha_out, *beta_out;
+};
+
+template <typename T, int N>
+struct alignas(sizeof(T) * N) Pack {
+    T v[N];
+};
+
+template <typename T> __device__ __forceinline__ T sign_one(uint32_t e);
+// +1 or -1 from the low bit of an entry (1 -> -1)
+template <> __device__ __forceinline__ float sign_one<float>(uint32_t e)
+{
+    return __uint_as_float(0x3f800000u | (e << 31));
+}
+template <> __device__ __forceinline__ double sign_one<double>(uint32_t e)
+{
+    return __hiloint2double((int)(0x3ff00000u | (e << 31)), 0);
+}
+
+template <typename E> __device__ __forceinline__ const E *ent_ptr(const SpinDev &s);
+template <> __device__ __forceinline__ const uint16_t *ent_ptr<uint16_t>(const SpinDev &s) { return s.e16; }
+template <> __device__ __forceinline__ const uint32_t *ent_ptr<uint32_t>(const SpinDev &s) { return s.e32; }
+
+// Record a_j, b_{j+1} and rotate the scalars (Algorithm 1 lines 7-11); called
+// by thread 0 of the last block of a norm-producing sweep.
+__device__ __forceinline__ void lanczos_rotate(LanczosScalars *S, double b2, double *alpha_out, double *beta_out)
+{
+    const double beta = sqrt(b2);
+    bool stop = false;
+    if (S->started > 0) {
+        const int j = S->j;
+        const double alpha = S->alpha;
+        alpha_out[j] = alpha;
+        beta_out[j] = beta;
+        const double amax = fmax(S->amax, fabs(alpha));
+        S->amax = amax;
+        S->j = j + 1;
+        stop = !isfinite(beta) || !(beta > S->tau * fmax(1.0, amax));      // lines 8-10, reading Q11
+    } else {
+        stop = !isfinite(beta) || !(beta > 0.0);                            // unusable start vector
+    }
+    if (stop) {
+        S->stop = 1;
+    } else {
+        S->c_prev = S->c_cur;
+        S->c_cur = 1.0 / beta;                                              // line 11, carried lazily
+        S->beta = beta;
+    }
+    S->started += 1;
+    S->ticket = 0;
+}
+
+// ------------------------------------------------------------------ the sweep
+// T: storage/arithmetic type.  R: rows (ROW) or columns (COL) per tile.
+// E: hop entry type.  VW: elements per global vector access of the COL sweep
+// (divides R; needs dim_dn % VW == 0).  COL: which sweep.  LZ: Lanczos form.
+template <typename T, int R, typename E, int VW, bool COL, bool LZ>
+__global__ void __launch_bounds__(kGatherThreads, 1)
+gather_sweep_kernel(GatherArgs<T> A)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ double red[32];
+    __shared__ int flag;
+    T *Xs = reinterpret_cast<T *>(smem_raw);              // [(n_in + 1)][R]
+    using PR = Pack<T, R>;
+    using PV = Pack<T, VW>;
+
+    const int64_t dd = A.dim_dn, du = A.dim_up;
+    const int n_in = (int)A.in.dim;
+    const int64_t n_out = COL ? dd : du;
+    const int64_t n_tiles = (n_out + R - 1) / R;
+    const E *__restrict__ ent = ent_ptr<E>(A.in);
+    const int64_t ld = A.in.ld;
+    const uint32_t pad = (uint32_t)n_in * 2u;
+    const T tt = (T)A.t, UU = (T)A.U;
+
+    T ac = T(0), c = T(1), bcp = T(0);
+    if (LZ) {
+        if (A.S->stop) return;
+        if (!COL) {
+            ac = (T)(A.S->alpha * A.S->c_cur);            // line 6: w = q_j - a_j f_j, f_j = c_j u_j
+        } else {
+            c = (T)A.S->c_cur;                            // f_{j+1} = c w
+            bcp = (T)(A.S->beta * A.S->c_prev);           // b_{j+1} f_j = (b_{j+1} c_j) u_j
+        }
+    }
+    if (threadIdx.x < R) Xs[(int64_t)n_in * R + threadIdx.x] = T(0);     // the zero slot
+    double racc = 0.0;                                    // |w|^2 (ROW) or q.f (COL) partial
+
+    for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        const int64_t o0 = tile * R;
+        const int nr = (int)min((int64_t)R, n_out - o0);
+        __syncthreads();                                  // gathers of the previous tile are done
+        // ---- stage the tile, interleaved
+        if (!COL) {
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                if (r < nr) {
+                    const int64_t J0 = (o0 + r) * dd;
+                    for (int b = threadIdx.x; b < n_in; b += kGatherThreads) {
+                        T v;
+                        if (LZ) {
+                            v = A.Q[J0 + b] - ac * A.F[J0 + b];
+                            A.Q[J0 + b] = v;
+                            racc += (double)v * (double)v;
+                        } else {
+                            v = A.x[J0 + b];
+                        }
+                        Xs[b * R + r] = v;
+                    }
+                } else {
+                    for (int b = threadIdx.x; b < n_in; b += kGatherThreads) Xs[b * R + r] = T(0);
+                }
+            }
+        } else {
+            const T *src = LZ ? A.Q : A.x;
+            if (nr == R) {
+                for (int a = threadIdx.x; a < n_in; a += kGatherThreads) {
+                    const T *p = src + (int64_t)a * dd + o0;
+                    PR v;
+#pragma unroll
+                    for (int q = 0; q < R / VW; ++q) {
+                        PV u = *reinterpret_cast<const PV *>(p + q * VW);
+#pragma unroll
+                        for (int e = 0; e < VW; ++e) v.v[q * VW + e] = u.v[e];
+                    }
+                    *reinterpret_cast<PR *>(Xs + a * R) = v;
+                }
+            } else {
+                for (int a = threadIdx.x; a < n_in; a += kGatherThreads) {
+                    const T *p = src + (int64_t)a * dd + o0;
+#pragma unroll
+                    for (int r = 0; r < R; ++r) Xs[a * R + r] = (r < nr) ? p[r] : T(0);
+                }
+            }
+        }
+        __syncthreads();
+
+        // ---- gather: one thread per contracted index i, R outputs each
+        uint32_t so[R];
+        if (!COL) {
+#pragma unroll
+            for (int r = 0; r < R; ++r) so[r] = (r < nr) ? A.st_out[o0 + r] : 0u;
+        }
+        for (int i = threadIdx.x; i < n_in; i += kGatherThreads) {
+            const int n = A.in.cnt[i];
+            T acc[R];
+#pragma unroll
+            for (int r = 0; r < R; ++r) acc[r] = T(0);
+            const E *ep = ent + i;
+            for (int k0 = 0; k0 < n; k0 += kGatherBatch) {
+                uint32_t e[kGatherBatch];
+#pragma unroll
+                for (int j = 0; j < kGatherBatch; ++j)
+                    e[j] = (k0 + j < n) ? (uint32_t)__ldg(ep + (int64_t)(k0 + j) * ld) : pad;
+#pragma unroll
+                for (int j = 0; j < kGatherBatch; ++j) {
+                    const PR v = *reinterpret_cast<const PR *>(Xs + (e[j] >> 1) * R);
+                    const T s = sign_one<T>(e[j]);
+#pragma unroll
+                    for (int r = 0; r < R; ++r) acc[r] = fma(s, v.v[r], acc[r]);
+                }
+            }
+            const PR xi = *reinterpret_cast<const PR *>(Xs + i * R);
+            if (!COL) {
+                // Algorithm 4: on-the-fly diagonal; one write per element
+                const uint32_t sd = A.in.st[i];
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    if (r < nr) {
+                        const T h = tt * acc[r] + UU * (T)__popc(so[r] & sd) * xi.v[r];
+                        const int64_t J = (o0 + r) * dd + i;
+                        if (LZ) A.Z[J] = h; else A.y[J] = h;
+                    }
+                }
+            } else {
+                const int64_t J = (int64_t)i * dd + o0;
+                if (nr == R) {
+#pragma unroll
+                    for (int q = 0; q < R / VW; ++q) {
+                        if (LZ) {
+                            PV f = *reinterpret_cast<const PV *>(A.F + J + q * VW);
+                            const PV z = *reinterpret_cast<const PV *>(A.Z + J + q * VW);
+#pragma unroll
+                            for (int e2 = 0; e2 < VW; ++e2) {
+                                const int r = q * VW + e2;
+                                const T qv = c * (tt * acc[r] + z.v[e2]) - bcp * f.v[e2];     // line 4 + eq. 13
+                                f.v[e2] = qv;
+                                racc += (double)qv * (double)(c * xi.v[r]);                     // line 5
+                            }
+                            *reinterpret_cast<PV *>(A.F + J + q * VW) = f;
+                        } else {
+                            PV yv = *reinterpret_cast<const PV *>(A.y + J + q * VW);
+#pragma unroll
+                            for (int e2 = 0; e2 < VW; ++e2) yv.v[e2] += tt * acc[q * VW + e2];
+                            *reinterpret_cast<PV *>(A.y + J + q * VW) = yv;
+                        }
+                    }
+                } else {
+#pragma unroll
+                    for (int r = 0; r < R; ++r) {
+                        if (r < nr) {
+                            if (LZ) {
+                                const T qv = c * (tt * acc[r] + A.Z[J + r]) - bcp * A.F[J + r];
+                                A.F[J + r] = qv;
+                                racc += (double)qv * (double)(c * xi.v[r]);
+                            } else {
+                                A.y[J + r] += tt * acc[r];
+                            }
+                        }
+                    }
+                }
+            }
+        }
+    }
+
+    if (LZ) {
+        const double sblk = block_sum(racc, red);
+        if (publish_and_check_last(sblk, A.partials, blockIdx.x, gridDim.x, &A.S->ticket, &flag)) {
+            const double tot = sum_partials(A.partials, gridDim.x, red);
+            if (threadIdx.x == 0) {
+                if (!COL) {
+                    lanczos_rotate(A.S, tot, A.alpha_out, A.beta_out);
+                } else {
+                    A.S->alpha = tot;
+                    A.S->ticket = 0;
+                }
+            }
+        }
+    }
+}
+
+// Closing sweep of a run: b_{m+1} = |q_m - a_m f_m| (Algorithm 1 lines 6-7) for
+// the last iteration, nothing written but the scalars.
+template <typename T>
+__global__ void __launch_bounds__(512)
+lanczos_final_norm_kernel(const T *__restrict__ Q, const T *__restrict__ F, int64_t dim, LanczosScalars *S,
+                          double *partials, double *alpha_out, double *beta_out)
+{
+    __shared__ double red[32];
+    __shared__ int flag;
+    if (S->stop) return;
+    const T ac = (T)(S->alpha * S->c_cur);
+    double acc = 0.0;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < dim; i += (int64_t)gridDim.x * blockDim.x) {
+        const T v = Q[i] - ac * F[i];
+        acc += (double)v * (double)v;
+    }
+    const double sblk = block_sum(acc, red);
+    if (publish_and_check_last(sblk, partials, blockIdx.x, gridDim.x, &S->ticket, &flag)) {
+        const double tot = sum_partials(partials, gridDim.x, red);
+        if (threadIdx.x == 0) lanczos_rotate(S, tot, alpha_out, beta_out);
+    }
+}
+
+__global__ void lanczos_scalars_init_kernel(LanczosScalars *S, double tau)
+{
+    S->c_cur = 0.0; S->c_prev = 0.0; S->beta = 0.0; S->alpha = 0.0; S->amax = 0.0; S->tau = tau;
+    S->j = 0; S->stop = 0; S->ticket = 0; S->started = 0;
+}
+
+}  // namespace hub

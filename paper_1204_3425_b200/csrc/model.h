@@ -27,7 +27,7 @@ struct LanczosScalars {
     int j;           // iterations completed
     int stop;        // breakdown (or bad start vector): later sweeps are no-ops
     unsigned ticket; // arrival counter of the sweep in flight
-    unsigned pad;
+    int started; // norm-producing sweeps finished (variant GATHER)
 };
 
 // Everything a kernel needs to know about the model (passed by value).
