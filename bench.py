@@ -42,7 +42,7 @@ def parse_args():
     p.add_argument("--dtype", default="both", choices=["f64", "f32", "both"])
     p.add_argument("--U", type=float, default=None)
     p.add_argument("--iters", type=int, default=None, help="Lanczos iterations per step (default: the config's)")
-    p.add_argument("--variant", default="auto", choices=["auto", "paper", "twosweep"])
+    p.add_argument("--variant", default="auto", choices=["auto", "paper", "twosweep", "gather"])
     p.add_argument("--no-cpu-baseline", action="store_true")
     p.add_argument("--no-e2e", action="store_true")
     return p.parse_args()
@@ -221,7 +221,8 @@ def run_native_dtype(args, cfg, U, dtype, rank, world, local):
     tdt = torch.float64 if dtype == "f64" else torch.float32
     s = 8 if dtype == "f64" else 4
     iters = args.iters or cfg.iters
-    variant = {"auto": hb.VARIANT_AUTO, "paper": hb.VARIANT_PAPER, "twosweep": hb.VARIANT_TWOSWEEP}[args.variant]
+    variant = {"auto": hb.VARIANT_AUTO, "paper": hb.VARIANT_PAPER, "twosweep": hb.VARIANT_TWOSWEEP,
+               "gather": hb.VARIANT_GATHER}[args.variant]
 
     m = hb.hubbard_create(cfg.n_sites, cfg.n_up, cfg.n_dn, cfg.bonds, cfg.t, U, dtype)
     m.hubbard_set_variant(variant)
@@ -264,8 +265,8 @@ def run_native_dtype(args, cfg, U, dtype, rank, world, local):
     for name, (n, tms) in ktimes.items():
         if n:
             kern[name] = {"launches": n, "avg_ms": tms / n}
-    hv_ms = sum(kern[k]["avg_ms"] for k in ("hv_paper", "row_sweep", "strip_sweep") if k in kern)
-    hv_parts = "+".join(k for k in ("hv_paper", "row_sweep", "strip_sweep") if k in kern)
+    hv_ms = sum(kern[k]["avg_ms"] for k in ("hv_paper", "row_sweep", "col_sweep") if k in kern)
+    hv_parts = "+".join(k for k in ("hv_paper", "row_sweep", "col_sweep") if k in kern)
     hv_bytes = 3 * cfg.dim * s                       # read f_j, read f_{j-1}, write q_j
     iter_ms = ms / (args.steps * iters)
     roof = {
@@ -278,7 +279,7 @@ def run_native_dtype(args, cfg, U, dtype, rank, world, local):
     roof["frac"] = roof["achieved"] / peak
     roof["whole_iteration"]["frac"] = roof["whole_iteration"]["achieved"] / peak
     for k, d in kern.items():
-        if k in ("row_sweep", "strip_sweep", "hv_paper", "axpy_norm"):
+        if k in ("row_sweep", "col_sweep", "hv_paper", "vec_sweep"):
             d["algorithmic_bytes"] = 3 * cfg.dim * s
             d["GBps"] = d["algorithmic_bytes"] / (d["avg_ms"] * 1e-3) / 1e9
 

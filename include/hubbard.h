@@ -60,8 +60,13 @@ enum {
 enum {
     HUBBARD_VARIANT_AUTO = 0,    /* library picks per model (default) */
     HUBBARD_VARIANT_PAPER = 1,   /* Algorithms 2-4 restated: one thread per element, one fused kernel */
-    HUBBARD_VARIANT_TWOSWEEP = 2 /* row sweep (down term + diagonal, row staged in shared memory)
+    HUBBARD_VARIANT_TWOSWEEP = 2,/* row sweep (down term + diagonal, row staged in shared memory)
                                     + strip sweep (up term over L2-resident column strips) */
+    HUBBARD_VARIANT_GATHER = 3   /* symmetric gather sweeps: R whole rows (down term) then R whole
+                                    columns (up term) staged interleaved in shared memory; in
+                                    lanczos_run the vector updates are folded into the two sweeps
+                                    (needs a third work vector).  INVALID if a row or column of V
+                                    does not fit in shared memory. */
 };
 
 /* ---- construction ("first, we prepare the data on the host") ----
@@ -126,7 +131,8 @@ int hubbard_apply(hubbard_model *m, const void *x_dev, void *y_dev, void *stream
  *               (Algorithm 1 lines 8-10, read as b_{j+1} <= tau*max(1,max_k|a_k|)
  *               or not finite, tau = 1e-10 for f64 / 1e-5 for f32; see
  *               lanczos_set_tau).
- * Work vectors (2 * dim elements) are allocated on first use and kept.
+ * Work vectors (2 * dim elements; 3 * dim for variant GATHER) are allocated on
+ * first use and kept.
  * The call enqueues everything on `stream`, then synchronises it and fills the
  * host arrays.  Errors: INVALID, DEVICE_OOM, CUDA, NO_DEVICE.
  */
@@ -171,9 +177,10 @@ int lanczos_ground_energy(const double *alpha, const double *beta, int m, double
  * bracketed by CUDA events on its stream; hubbard_kernel_times then returns,
  * per kernel class, the number of launches and the summed device time in ms
  * since the last hubbard_profile call (it synchronises the recorded events).
- * Classes: 0 = H v kernel(s) of variant PAPER, 1 = row sweep, 2 = strip sweep,
- * 3 = Lanczos axpy+norm sweep, 4 = scalar/finalise kernels, 5 = setup (copy,
- * initial norm).  Arrays have HUBBARD_N_KCLASS entries.
+ * Classes: 0 = H v kernel(s) of variant PAPER, 1 = row sweep (down term),
+ * 2 = strip / column sweep (up term), 3 = Lanczos axpy+norm or closing norm
+ * sweep, 4 = scalar/finalise kernels, 5 = setup (copy, initial norm).
+ * Arrays have HUBBARD_N_KCLASS entries.
  * hubbard_launch_count: kernels launched by this model since creation. */
 #define HUBBARD_N_KCLASS 6
 int hubbard_profile(hubbard_model *m, int enable);

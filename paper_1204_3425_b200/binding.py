@@ -13,9 +13,9 @@ import numpy as np
 from . import build as _build
 
 HUBBARD_F32, HUBBARD_F64 = 0, 1
-VARIANT_AUTO, VARIANT_PAPER, VARIANT_TWOSWEEP = 0, 1, 2
+VARIANT_AUTO, VARIANT_PAPER, VARIANT_TWOSWEEP, VARIANT_GATHER = 0, 1, 2, 3
 N_KCLASS = 6
-KCLASS_NAMES = ("hv_paper", "row_sweep", "strip_sweep", "axpy_norm", "scalar", "setup")
+KCLASS_NAMES = ("hv_paper", "row_sweep", "col_sweep", "vec_sweep", "scalar", "setup")
 
 ABI_SYMBOLS = (
     "hubbard_create", "hubbard_create_host", "hubbard_destroy", "hubbard_dims", "hubbard_set_U",

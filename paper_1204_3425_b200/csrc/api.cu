@@ -5,6 +5,7 @@
 #include <cstring>
 #include <new>
 
+#include "kernels_gather.cuh"
 #include "kernels_lanczos.cuh"
 #include "kernels_paper.cuh"
 #include "kernels_twosweep.cuh"
@@ -65,6 +66,38 @@ int build_host(hubbard_model **out, int n_sites, int n_up, int n_dn, const int32
     return HUBBARD_OK;
 }
 
+// Column-major ELL of one spin for variant GATHER (kernels_gather.cuh).
+int upload_gather_table(hubbard_model *m, const SpinTable &tab, const uint32_t *d_states, SpinDev *out)
+{
+    SpinDev G{};
+    G.dim = tab.dim;
+    G.w = (std::max(tab.width, 1) + 7) / 8 * 8;
+    G.ld = (tab.dim + 31) / 32 * 32;
+    G.st = d_states;
+    const uint32_t pad = (uint32_t)tab.dim * 2u;
+    std::vector<uint32_t> e32((size_t)G.ld * G.w, pad);
+    std::vector<int32_t> cnt((size_t)tab.dim);
+    for (int64_t r = 0; r < tab.dim; ++r) {
+        int n = (int)(tab.rowptr[r + 1] - tab.rowptr[r]);
+        cnt[(size_t)r] = n;
+        for (int k = 0; k < n; ++k) {
+            size_t s = (size_t)(tab.rowptr[r] + k);
+            e32[((size_t)(k / 8) * G.ld + r) * 8 + k % 8] = (uint32_t)tab.col[s] * 2u + (tab.plus[s] ? 0u : 1u);
+        }
+    }
+    int rc;
+    if ((rc = dev_upload(m, e32, &G.e32))) return rc;
+    if ((rc = dev_upload(m, cnt, &G.cnt))) return rc;
+    G.e16 = nullptr;
+    if (tab.dim + 1 <= 32768) {
+        std::vector<uint16_t> e16(e32.size());
+        for (size_t i = 0; i < e32.size(); ++i) e16[i] = (uint16_t)e32[i];
+        if ((rc = dev_upload(m, e16, &G.e16))) return rc;
+    }
+    *out = G;
+    return HUBBARD_OK;
+}
+
 // Device layouts of the two hop tables (see model.h / DESIGN.md "data layout").
 int upload_tables(hubbard_model *m)
 {
@@ -110,6 +143,9 @@ int upload_tables(hubbard_model *m)
             for (size_t i = 0; i < de.size(); ++i) d16[i] = (uint16_t)de[i];
             if ((rc = dev_upload(m, d16, &D.dn_ent16))) return rc;
         }
+        // variant GATHER: both spins column-major, entry = col * 2 + neg
+        if ((rc = upload_gather_table(m, m->up, D.st_up, &D.g_up))) return rc;
+        if ((rc = upload_gather_table(m, m->dn, D.st_dn, &D.g_dn))) return rc;
     } catch (const std::bad_alloc &) {
         return HUBBARD_ERR_HOST_OOM;
     }
@@ -170,10 +206,77 @@ int ensure_partials(hubbard_model *m, int64_t n)
     return HUBBARD_OK;
 }
 
+// Largest tile height R (rows or columns per tile) of variant GATHER for a
+// contracted dimension n_in, 0 if even R = 1 does not fit in shared memory.
+int gather_R(const hubbard_model *m, int64_t n_in)
+{
+    const size_t es = m->dtype == HUBBARD_F32 ? 4 : 8;
+    const size_t budget = (size_t)std::max(0, m->max_smem_optin - 1024);
+    int forced = env_int("HUBBARD_GATHER_R", 0);
+    for (int R = (int)(16 / es); R >= 1; R >>= 1) {
+        if (forced > 0 && R > forced) continue;
+        if ((size_t)(n_in + 1) * R * es <= budget) return R;
+    }
+    return 0;
+}
+
+bool gather_fits(const hubbard_model *m) { return gather_R(m, m->dn.dim) > 0 && gather_R(m, m->up.dim) > 0; }
+
 int resolve_variant(const hubbard_model *m)
 {
     if (m->variant != HUBBARD_VARIANT_AUTO) return m->variant;
-    return (m->dn.dim >= 512) ? HUBBARD_VARIANT_TWOSWEEP : HUBBARD_VARIANT_PAPER;
+    if (m->dn.dim < 512 || m->up.dim < 512) return HUBBARD_VARIANT_PAPER;
+    return gather_fits(m) ? HUBBARD_VARIANT_GATHER : HUBBARD_VARIANT_TWOSWEEP;
+}
+
+// ---- variant GATHER
+template <typename T, int R, typename E, int VW, bool COL, bool LZ>
+int launch_gather_inst(hubbard_model *m, const GatherArgs<T> &A, cudaStream_t st)
+{
+    auto kern = gather_sweep_kernel<T, R, E, VW, COL, LZ>;
+    const size_t smem = (size_t)(A.in.dim + 1) * R * sizeof(T);
+    CU_TRY(m, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const int64_t n_out = COL ? A.dim_dn : A.dim_up;
+    const int64_t tiles = (n_out + R - 1) / R;
+    const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(tiles, m->sm_count));
+    ProfScope ps(m, COL ? 2 : 1, st);
+    kern<<<grid, kGatherThreads, smem, st>>>(A);
+    return after_launch(m);
+}
+
+template <typename T, int R, typename E, bool COL, bool LZ>
+int launch_gather_vw(hubbard_model *m, const GatherArgs<T> &A, cudaStream_t st)
+{
+    if constexpr (!COL) {
+        return launch_gather_inst<T, R, E, 1, false, LZ>(m, A, st);
+    } else {
+        int vw = R;
+        while (vw > 1 && (A.dim_dn % vw) != 0) vw >>= 1;
+        if constexpr (R >= 4) if (vw == 4) return launch_gather_inst<T, R, E, 4, true, LZ>(m, A, st);
+        if constexpr (R >= 2) if (vw >= 2) return launch_gather_inst<T, R, E, 2, true, LZ>(m, A, st);
+        return launch_gather_inst<T, R, E, 1, true, LZ>(m, A, st);
+    }
+}
+
+template <typename T, bool COL, bool LZ>
+int launch_gather(hubbard_model *m, GatherArgs<T> A, cudaStream_t st)
+{
+    const DevModel &D = m->dev;
+    A.in = COL ? D.g_up : D.g_dn;
+    A.st_out = D.st_up;
+    A.dim_up = D.dim_up; A.dim_dn = D.dim_dn; A.t = m->t; A.U = m->U;
+    const int R = gather_R(m, A.in.dim);
+    if (R == 0) return HUBBARD_ERR_INVALID;
+    if (LZ) { int rc = ensure_partials(m, m->sm_count); if (rc) return rc; A.partials = m->d_partial; }
+    if (!A.in.e16) {
+        if constexpr (sizeof(T) == 4) return launch_gather_vw<T, 1, uint32_t, COL, LZ>(m, A, st);
+        return HUBBARD_ERR_INVALID;      // dim >= 32767 never fits in shared memory at 8 bytes/element
+    }
+    if constexpr (sizeof(T) == 4) {
+        if (R == 4) return launch_gather_vw<T, 4, uint16_t, COL, LZ>(m, A, st);
+    }
+    if (R >= 2) return launch_gather_vw<T, 2, uint16_t, COL, LZ>(m, A, st);
+    return launch_gather_vw<T, 1, uint16_t, COL, LZ>(m, A, st);
 }
 
 // ---- variant PAPER
@@ -275,7 +378,16 @@ template <typename T, bool LZ>
 int apply_impl(hubbard_model *m, const T *x, T *y, cudaStream_t st)
 {
     m->dev.U = m->U;
-    if (resolve_variant(m) == HUBBARD_VARIANT_PAPER) return launch_paper<T, LZ>(m, x, y, st);
+    const int variant = resolve_variant(m);
+    if (variant == HUBBARD_VARIANT_PAPER) return launch_paper<T, LZ>(m, x, y, st);
+    if (variant == HUBBARD_VARIANT_GATHER) {
+        if (LZ) return HUBBARD_ERR_INVALID;          // the Lanczos form of GATHER is lanczos_gather_impl
+        GatherArgs<T> G{};
+        G.x = x; G.y = y;
+        int rc = launch_gather<T, false, false>(m, G, st);
+        if (rc) return rc;
+        return launch_gather<T, true, false>(m, G, st);
+    }
     SweepArgs<T> A{x, y, LZ ? m->d_scal : nullptr, m->d_partial};
     int rc = m->dev.dn_ent16 ? launch_row<T, uint16_t, LZ>(m, A, m->dev.dn_ent16, st)
                              : launch_row<T, uint32_t, LZ>(m, A, m->dev.dn_ent32, st);
@@ -288,10 +400,10 @@ int apply_impl(hubbard_model *m, const T *x, T *y, cudaStream_t st)
 // --------------------------------------------------------------- Lanczos run
 namespace {
 
-int ensure_lanczos_state(hubbard_model *m, int iters)
+int ensure_lanczos_state(hubbard_model *m, int iters, int n_vec)
 {
     const size_t bytes = (size_t)model_dim(m) * elem_size(m);
-    for (int i = 0; i < 2; ++i)
+    for (int i = 0; i < n_vec; ++i)
         if (!m->work[i]) CU_TRY(m, cudaMalloc(&m->work[i], std::max<size_t>(bytes, 16)));
     if (!m->d_scal) CU_TRY(m, cudaMalloc((void **)&m->d_scal, sizeof(LanczosScalars)));
     if (iters > m->coef_cap) {
@@ -306,11 +418,62 @@ int ensure_lanczos_state(hubbard_model *m, int iters)
     return HUBBARD_OK;
 }
 
+int fetch_coefficients(hubbard_model *m, int iters, double *alpha, double *beta, int *done, cudaStream_t st)
+{
+    LanczosScalars h{};
+    CU_TRY(m, cudaMemcpyAsync(&h, m->d_scal, sizeof(h), cudaMemcpyDeviceToHost, st));
+    CU_TRY(m, cudaStreamSynchronize(st));
+    int n = std::max(0, std::min(h.j, iters));
+    if (n > 0) {
+        CU_TRY(m, cudaMemcpy(alpha, m->d_alpha, (size_t)n * sizeof(double), cudaMemcpyDeviceToHost));
+        CU_TRY(m, cudaMemcpy(beta, m->d_beta, (size_t)n * sizeof(double), cudaMemcpyDeviceToHost));
+    }
+    if (done) *done = n;
+    return HUBBARD_OK;
+}
+
+// Variant GATHER: two sweeps per iteration, vector updates folded in
+// (kernels_gather.cuh), one closing norm sweep for b_{m+1}.
+template <typename T>
+int lanczos_gather_impl(hubbard_model *m, const T *v0, int iters, double *alpha, double *beta, int *done,
+                        cudaStream_t st)
+{
+    const int64_t dim = model_dim(m);
+    int rc = ensure_lanczos_state(m, iters, 3);
+    if (rc) return rc;
+    const int vec_grid = (int)std::max<int64_t>(1, std::min<int64_t>((int64_t)m->sm_count * 4, (dim + 2047) / 2048));
+    if ((rc = ensure_partials(m, std::max(vec_grid, m->sm_count)))) return rc;
+    T *Q = static_cast<T *>(m->work[0]), *F = static_cast<T *>(m->work[1]), *Z = static_cast<T *>(m->work[2]);
+    const double tau = m->tau >= 0 ? m->tau : (m->dtype == HUBBARD_F64 ? 1e-10 : 1e-5);
+    {
+        ProfScope ps(m, 5, st);
+        CU_TRY(m, cudaMemcpyAsync(Q, v0, (size_t)dim * sizeof(T), cudaMemcpyDeviceToDevice, st));   // "q_0" = f_1 unnormalised
+        CU_TRY(m, cudaMemsetAsync(F, 0, (size_t)dim * sizeof(T), st));                              // line 2: f_0 <- 0
+        lanczos_scalars_init_kernel<<<1, 1, 0, st>>>(m->d_scal, tau);                               // line 1: b_1 <- 0
+        if ((rc = after_launch(m))) return rc;
+    }
+    GatherArgs<T> G{};
+    G.S = m->d_scal; G.Z = Z; G.alpha_out = m->d_alpha; G.beta_out = m->d_beta;
+    for (int j = 0; j < iters; ++j) {
+        G.Q = Q; G.F = F;
+        if ((rc = launch_gather<T, false, true>(m, G, st))) return rc;     // lines 6-11 of j-1, row half of line 4
+        if ((rc = launch_gather<T, true, true>(m, G, st))) return rc;      // line 4 (+ eq. 13), line 5
+        std::swap(Q, F);
+    }
+    {
+        ProfScope ps(m, 3, st);
+        lanczos_final_norm_kernel<T><<<vec_grid, 512, 0, st>>>(Q, F, dim, m->d_scal, m->d_partial, m->d_alpha, m->d_beta);
+        if ((rc = after_launch(m))) return rc;
+    }
+    return fetch_coefficients(m, iters, alpha, beta, done, st);
+}
+
 template <typename T>
 int lanczos_impl(hubbard_model *m, const T *v0, int iters, double *alpha, double *beta, int *done, cudaStream_t st)
 {
     const int64_t dim = model_dim(m);
-    int rc = ensure_lanczos_state(m, iters);
+    if (resolve_variant(m) == HUBBARD_VARIANT_GATHER) return lanczos_gather_impl<T>(m, v0, iters, alpha, beta, done, st);
+    int rc = ensure_lanczos_state(m, iters, 2);
     if (rc) return rc;
     const int vec_grid = (int)std::max<int64_t>(1, std::min<int64_t>((int64_t)m->sm_count * 4, (dim + 2047) / 2048));
     if ((rc = ensure_partials(m, vec_grid))) return rc;
@@ -335,16 +498,7 @@ int lanczos_impl(hubbard_model *m, const T *v0, int iters, double *alpha, double
         }
         std::swap(cur, prev);
     }
-    LanczosScalars h{};
-    CU_TRY(m, cudaMemcpyAsync(&h, m->d_scal, sizeof(h), cudaMemcpyDeviceToHost, st));
-    CU_TRY(m, cudaStreamSynchronize(st));
-    int n = std::max(0, std::min(h.j, iters));
-    if (n > 0) {
-        CU_TRY(m, cudaMemcpy(alpha, m->d_alpha, (size_t)n * sizeof(double), cudaMemcpyDeviceToHost));
-        CU_TRY(m, cudaMemcpy(beta, m->d_beta, (size_t)n * sizeof(double), cudaMemcpyDeviceToHost));
-    }
-    if (done) *done = n;
-    return HUBBARD_OK;
+    return fetch_coefficients(m, iters, alpha, beta, done, st);
 }
 
 int ensure_stage(hubbard_model *m, int which)
@@ -396,7 +550,8 @@ void hubbard_destroy(hubbard_model *m)
     if (!m) return;
     for (auto &r : m->prof) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
     for (void *p : m->dev_allocs) cudaFree(p);
-    for (int i = 0; i < 2; ++i) { if (m->work[i]) cudaFree(m->work[i]); if (m->stage[i]) cudaFree(m->stage[i]); }
+    for (int i = 0; i < 3; ++i) if (m->work[i]) cudaFree(m->work[i]);
+    for (int i = 0; i < 2; ++i) if (m->stage[i]) cudaFree(m->stage[i]);
     if (m->d_scal) cudaFree(m->d_scal);
     if (m->d_partial) cudaFree(m->d_partial);
     if (m->d_alpha) cudaFree(m->d_alpha);
@@ -422,7 +577,8 @@ int hubbard_set_U(hubbard_model *m, double U)
 
 int hubbard_set_variant(hubbard_model *m, int variant)
 {
-    if (!m || variant < HUBBARD_VARIANT_AUTO || variant > HUBBARD_VARIANT_TWOSWEEP) return HUBBARD_ERR_INVALID;
+    if (!m || variant < HUBBARD_VARIANT_AUTO || variant > HUBBARD_VARIANT_GATHER) return HUBBARD_ERR_INVALID;
+    if (variant == HUBBARD_VARIANT_GATHER && m->has_device && !gather_fits(m)) return HUBBARD_ERR_INVALID;
     m->variant = variant;
     return HUBBARD_OK;
 }

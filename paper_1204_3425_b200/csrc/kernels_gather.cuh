@@ -11,8 +11,10 @@
 // index, r = 0..R-1 the tile's rows/columns), R*sizeof(T) = 16 bytes when it
 // fits, so that ONE 128-bit shared-memory load fetches the hop source of all R
 // outputs a thread owns; the hop entry (Algorithms 2/3: Aj, Ax of the ELL
-// format, column-major so that a warp reads them coalesced)
-// is read once per R outputs.  Padding entries point at a zero slot.
+// format, stored so that a warp reads them coalesced: batches
+// of 8 entries of one state are contiguous, batch kb of state i at
+// [(kb * ld + i) * 8]) is read once per R outputs.  Padding entries point at a
+// zero slot.
 //
 // Lanczos form (Algorithm 1 with eq. 13), 8 vector passes per
 // iteration, no separate axpy/norm kernel:
@@ -29,19 +31,6 @@ namespace hub {
 
 constexpr int kGatherThreads = 1024;
 constexpr int kGatherBatch = 8;          // hop entries fetched ahead per thread
-
-// One spin's hop table in the device layout of this variant: column-major ELL
-// [w][ld], entry = col * 2 + neg, the matrix element being t * (neg ? -1 : +1)
-// (PAPER.md:99-104); padding entries are dim * 2 (the zero slot, sign +).
-struct SpinDev {
-    int64_t dim;            // dim_sigma
-    int64_t ld;             // leading dimension of the ELL arrays (multiple of 32)
-    int w;                  // ELL width
-    const uint16_t *e16;    // entries when dim + 1 <= 32768, else null
-    const uint32_t *e32;    // entries (always present)
-    const int32_t *cnt;     // hops per state
-    const uint32_t *st;     // basis bit patterns
-};
 
 template <typename T>
 struct GatherArgs {
@@ -73,6 +62,28 @@ template <> __device__ __forceinline__ float sign_one<float>(uint32_t e)
 template <> __device__ __forceinline__ double sign_one<double>(uint32_t e)
 {
     return __hiloint2double((int)(0x3ff00000u | (e << 31)), 0);
+}
+
+// One batch of kGatherBatch hop entries of one state: 16 (uint16) or 32 (uint32)
+// contiguous bytes, read through the read-only path.
+__device__ __forceinline__ Pack<uint16_t, 8> load_batch(const Pack<uint16_t, 8> *p)
+{
+    const uint4 u = __ldg(reinterpret_cast<const uint4 *>(p));
+    Pack<uint16_t, 8> o;
+    o.v[0] = (uint16_t)(u.x & 0xffffu); o.v[1] = (uint16_t)(u.x >> 16);
+    o.v[2] = (uint16_t)(u.y & 0xffffu); o.v[3] = (uint16_t)(u.y >> 16);
+    o.v[4] = (uint16_t)(u.z & 0xffffu); o.v[5] = (uint16_t)(u.z >> 16);
+    o.v[6] = (uint16_t)(u.w & 0xffffu); o.v[7] = (uint16_t)(u.w >> 16);
+    return o;
+}
+__device__ __forceinline__ Pack<uint32_t, 8> load_batch(const Pack<uint32_t, 8> *p)
+{
+    const uint4 a = __ldg(reinterpret_cast<const uint4 *>(p));
+    const uint4 b = __ldg(reinterpret_cast<const uint4 *>(p) + 1);
+    Pack<uint32_t, 8> o;
+    o.v[0] = a.x; o.v[1] = a.y; o.v[2] = a.z; o.v[3] = a.w;
+    o.v[4] = b.x; o.v[5] = b.y; o.v[6] = b.z; o.v[7] = b.w;
+    return o;
 }
 
 template <typename E> __device__ __forceinline__ const E *ent_ptr(const SpinDev &s);
@@ -122,6 +133,8 @@ gather_sweep_kernel(GatherArgs<T> A)
     T *Xs = reinterpret_cast<T *>(smem_raw);              // [(n_in + 1)][R]
     using PR = Pack<T, R>;
     using PV = Pack<T, VW>;
+    using EB = Pack<E, kGatherBatch>;
+    const unsigned char *xs_bytes = smem_raw;
 
     const int64_t dd = A.dim_dn, du = A.dim_up;
     const int n_in = (int)A.in.dim;
@@ -129,7 +142,6 @@ gather_sweep_kernel(GatherArgs<T> A)
     const int64_t n_tiles = (n_out + R - 1) / R;
     const E *__restrict__ ent = ent_ptr<E>(A.in);
     const int64_t ld = A.in.ld;
-    const uint32_t pad = (uint32_t)n_in * 2u;
     const T tt = (T)A.t, UU = (T)A.U;
 
     T ac = T(0), c = T(1), bcp = T(0);
@@ -205,19 +217,21 @@ gather_sweep_kernel(GatherArgs<T> A)
             T acc[R];
 #pragma unroll
             for (int r = 0; r < R; ++r) acc[r] = T(0);
-            const E *ep = ent + i;
+            const EB *ep = reinterpret_cast<const EB *>(ent) + i;
+            EB pk = load_batch(ep);                       // every state has at least one (padding) batch
             for (int k0 = 0; k0 < n; k0 += kGatherBatch) {
-                uint32_t e[kGatherBatch];
-#pragma unroll
-                for (int j = 0; j < kGatherBatch; ++j)
-                    e[j] = (k0 + j < n) ? (uint32_t)__ldg(ep + (int64_t)(k0 + j) * ld) : pad;
+                ep += ld;
+                EB nxt = pk;
+                if (k0 + kGatherBatch < n) nxt = load_batch(ep);        // fetch ahead: hides the L2 latency
 #pragma unroll
                 for (int j = 0; j < kGatherBatch; ++j) {
-                    const PR v = *reinterpret_cast<const PR *>(Xs + (e[j] >> 1) * R);
-                    const T s = sign_one<T>(e[j]);
+                    const uint32_t e = pk.v[j];
+                    const PR v = *reinterpret_cast<const PR *>(xs_bytes + (e & ~1u) * (uint32_t)(sizeof(PR) / 2));
+                    const T s = sign_one<T>(e);
 #pragma unroll
                     for (int r = 0; r < R; ++r) acc[r] = fma(s, v.v[r], acc[r]);
                 }
+                pk = nxt;
             }
             const PR xi = *reinterpret_cast<const PR *>(Xs + i * R);
             if (!COL) {

@@ -30,6 +30,20 @@ struct LanczosScalars {
     int started; // norm-producing sweeps finished (variant GATHER)
 };
 
+// One spin's hop table in the device layout of this variant: column-major ELL
+// [w][ld], entry = col * 2 + neg, the matrix element being t * (neg ? -1 : +1)
+// (PAPER.md:99-104); padding entries are dim * 2 (the zero slot, sign +).
+struct SpinDev {
+    int64_t dim;            // dim_sigma
+    int64_t ld;             // states per batch plane (multiple of 32): entry k of state i
+                            // sits at [((k / 8) * ld + i) * 8 + k % 8]
+    int w;                  // ELL width rounded up to a multiple of 8
+    const uint16_t *e16;    // entries when dim + 1 <= 32768, else null
+    const uint32_t *e32;    // entries (always present)
+    const int32_t *cnt;     // hops per state
+    const uint32_t *st;     // basis bit patterns
+};
+
 // Everything a kernel needs to know about the model (passed by value).
 struct DevModel {
     int64_t dim_up, dim_dn;
@@ -45,6 +59,7 @@ struct DevModel {
     int w_dn;
     int64_t ld_dn;
     double t, U;
+    SpinDev g_up, g_dn;                  // tables of variant GATHER
 };
 
 struct ProfRecord {
@@ -70,7 +85,7 @@ struct hubbard_model {
     hub::DevModel dev{};
     std::vector<void *> dev_allocs;    // everything to cudaFree
     // Lanczos state (allocated on first use)
-    void *work[2] = {nullptr, nullptr};
+    void *work[3] = {nullptr, nullptr, nullptr};   // third vector: variant GATHER only
     hub::LanczosScalars *d_scal = nullptr;
     double *d_partial = nullptr;       // per-block partial sums
     int64_t n_partial = 0;

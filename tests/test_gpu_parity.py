@@ -21,7 +21,8 @@ pytestmark = pytest.mark.gpu
 TOL_HV = {"f64": 1e-12, "f32": 1e-5}
 TOL_E0 = {"f64": 1e-10, "f32": 1e-5}
 TDT = {"f64": torch.float64, "f32": torch.float32}
-VARIANTS = {"paper": hb.VARIANT_PAPER, "twosweep": hb.VARIANT_TWOSWEEP, "auto": hb.VARIANT_AUTO}
+VARIANTS = {"paper": hb.VARIANT_PAPER, "twosweep": hb.VARIANT_TWOSWEEP, "gather": hb.VARIANT_GATHER,
+            "auto": hb.VARIANT_AUTO}
 
 
 def dev():
@@ -58,7 +59,7 @@ SMALL = [
 ]
 
 
-@pytest.mark.parametrize("variant", ["paper", "twosweep"])
+@pytest.mark.parametrize("variant", ["paper", "twosweep", "gather"])
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 @pytest.mark.parametrize("ns,nu,nd,bonds", SMALL)
 def test_apply_vs_definition_small(ns, nu, nd, bonds, dtype, variant):
@@ -81,7 +82,7 @@ def test_apply_vs_definition_small(ns, nu, nd, bonds, dtype, variant):
         assert rel_max_err(y, y_ref) <= TOL_HV[dtype]
 
 
-@pytest.mark.parametrize("variant", ["paper", "twosweep"])
+@pytest.mark.parametrize("variant", ["paper", "twosweep", "gather"])
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 @pytest.mark.parametrize("name", ["C1", "C2", "C3"])
 def test_apply_full_vector_C1_C2_C3(name, dtype, variant):
@@ -223,13 +224,13 @@ def _lanczos_case(name, U, dtype, variant, iters, n_prefix):
     return e_gpu
 
 
-@pytest.mark.parametrize("variant", ["paper", "twosweep"])
+@pytest.mark.parametrize("variant", ["paper", "twosweep", "gather"])
 def test_lanczos_C1(variant):
     e = _lanczos_case("C1", 4.0, "f64", variant, 100, 50)
     assert abs(e - (-4.603526299989)) < 1e-9          # SURVEY P11, also dense eigvalsh in the CPU suite
 
 
-@pytest.mark.parametrize("variant", ["paper", "twosweep"])
+@pytest.mark.parametrize("variant", ["paper", "twosweep", "gather"])
 @pytest.mark.parametrize("dtype,n_prefix", [("f64", 50), ("f32", 30)])
 @pytest.mark.parametrize("U", [4.0, 8.0])
 def test_lanczos_C2(U, dtype, n_prefix, variant):
@@ -270,7 +271,7 @@ def test_lanczos_breakdown_atomic_limit():
     Q11) exactly where the oracle does."""
     ns, nu, nd, bonds = 6, 3, 3, ring_bonds(6)
     ref = RefModel(ns, nu, nd, bonds, 0.0, 4.0)
-    for variant in ("paper", "twosweep"):
+    for variant in ("paper", "twosweep", "gather"):
         m = hb.hubbard_create(ns, nu, nd, bonds, 0.0, 4.0, "f64")
         m.hubbard_set_variant(VARIANTS[variant])
         v0, v0_np = start_vector(5, m.dim, "f64")
