@@ -65,7 +65,7 @@ enum {
     HUBBARD_VARIANT_GATHER = 3   /* symmetric gather sweeps: R whole rows (down term) then R whole
                                     columns (up term) staged interleaved in shared memory; in
                                     lanczos_run the vector updates are folded into the two sweeps
-                                    (needs a third work vector).  INVALID if a row or column of V
+                                    (five work vectors in tile-major layouts).  INVALID if a row or column of V
                                     does not fit in shared memory. */
 };
 
@@ -131,7 +131,7 @@ int hubbard_apply(hubbard_model *m, const void *x_dev, void *y_dev, void *stream
  *               (Algorithm 1 lines 8-10, read as b_{j+1} <= tau*max(1,max_k|a_k|)
  *               or not finite, tau = 1e-10 for f64 / 1e-5 for f32; see
  *               lanczos_set_tau).
- * Work vectors (2 * dim elements; 3 * dim for variant GATHER) are allocated on
+ * Work vectors (2 * dim elements; 5 * dim for variant GATHER) are allocated on
  * first use and kept.
  * The call enqueues everything on `stream`, then synchronises it and fills the
  * host arrays.  Errors: INVALID, DEVICE_OOM, CUDA, NO_DEVICE.

@@ -206,21 +206,32 @@ int ensure_partials(hubbard_model *m, int64_t n)
     return HUBBARD_OK;
 }
 
-// Largest tile height R (rows or columns per tile) of variant GATHER for a
-// contracted dimension n_in, 0 if even R = 1 does not fit in shared memory.
-int gather_R(const hubbard_model *m, int64_t n_in)
+// Tile height R (rows per ROW tile = columns per COL tile) of variant GATHER:
+// the largest R with R * sizeof(T) <= 16 for which a whole row AND a whole
+// column of V fit in shared memory; 0 if even R = 1 does not fit.
+int gather_R(const hubbard_model *m)
 {
     const size_t es = m->dtype == HUBBARD_F32 ? 4 : 8;
     const size_t budget = (size_t)std::max(0, m->max_smem_optin - 1024);
+    const int64_t n_in = std::max(m->dn.dim, m->up.dim);
     int forced = env_int("HUBBARD_GATHER_R", 0);
     for (int R = (int)(16 / es); R >= 1; R >>= 1) {
         if (forced > 0 && R > forced) continue;
-        if ((size_t)(n_in + 1) * R * es <= budget) return R;
+        if ((size_t)(n_in + R + 1) * R * es <= budget) return R;
     }
     return 0;
 }
 
-bool gather_fits(const hubbard_model *m) { return gather_R(m, m->dn.dim) > 0 && gather_R(m, m->up.dim) > 0; }
+bool gather_fits(const hubbard_model *m) { return gather_R(m) > 0; }
+
+int64_t round_up(int64_t n, int64_t r) { return (n + r - 1) / r * r; }
+
+// elements of one work vector of variant GATHER (either tile-major layout)
+int64_t gather_vec_elems(const hubbard_model *m)
+{
+    const int R = std::max(1, gather_R(m));
+    return round_up(m->up.dim, R) * round_up(m->dn.dim, R);
+}
 
 int resolve_variant(const hubbard_model *m)
 {
@@ -230,32 +241,20 @@ int resolve_variant(const hubbard_model *m)
 }
 
 // ---- variant GATHER
-template <typename T, int R, typename E, int VW, bool COL, bool LZ>
-int launch_gather_inst(hubbard_model *m, const GatherArgs<T> &A, cudaStream_t st)
+template <typename T, int R, typename E, bool COL, bool LZ>
+int launch_gather_inst(hubbard_model *m, GatherArgs<T> A, cudaStream_t st)
 {
-    auto kern = gather_sweep_kernel<T, R, E, VW, COL, LZ>;
-    const size_t smem = (size_t)(A.in.dim + 1) * R * sizeof(T);
+    auto kern = gather_sweep_kernel<T, R, E, COL, LZ>;
+    A.du_p = round_up(A.dim_up, R);
+    A.dd_p = round_up(A.dim_dn, R);
+    const int64_t n_in_p = COL ? A.du_p : A.dd_p;
+    const size_t smem = (size_t)(n_in_p + 1) * R * sizeof(T);
     CU_TRY(m, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    const int64_t n_out = COL ? A.dim_dn : A.dim_up;
-    const int64_t tiles = (n_out + R - 1) / R;
+    const int64_t tiles = (COL ? A.dd_p : A.du_p) / R;
     const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(tiles, m->sm_count));
     ProfScope ps(m, COL ? 2 : 1, st);
     kern<<<grid, kGatherThreads, smem, st>>>(A);
     return after_launch(m);
-}
-
-template <typename T, int R, typename E, bool COL, bool LZ>
-int launch_gather_vw(hubbard_model *m, const GatherArgs<T> &A, cudaStream_t st)
-{
-    if constexpr (!COL) {
-        return launch_gather_inst<T, R, E, 1, false, LZ>(m, A, st);
-    } else {
-        int vw = R;
-        while (vw > 1 && (A.dim_dn % vw) != 0) vw >>= 1;
-        if constexpr (R >= 4) if (vw == 4) return launch_gather_inst<T, R, E, 4, true, LZ>(m, A, st);
-        if constexpr (R >= 2) if (vw >= 2) return launch_gather_inst<T, R, E, 2, true, LZ>(m, A, st);
-        return launch_gather_inst<T, R, E, 1, true, LZ>(m, A, st);
-    }
 }
 
 template <typename T, bool COL, bool LZ>
@@ -265,18 +264,47 @@ int launch_gather(hubbard_model *m, GatherArgs<T> A, cudaStream_t st)
     A.in = COL ? D.g_up : D.g_dn;
     A.st_out = D.st_up;
     A.dim_up = D.dim_up; A.dim_dn = D.dim_dn; A.t = m->t; A.U = m->U;
-    const int R = gather_R(m, A.in.dim);
+    const int R = gather_R(m);
     if (R == 0) return HUBBARD_ERR_INVALID;
     if (LZ) { int rc = ensure_partials(m, m->sm_count); if (rc) return rc; A.partials = m->d_partial; }
     if (!A.in.e16) {
-        if constexpr (sizeof(T) == 4) return launch_gather_vw<T, 1, uint32_t, COL, LZ>(m, A, st);
-        return HUBBARD_ERR_INVALID;      // dim >= 32767 never fits in shared memory at 8 bytes/element
+        if constexpr (sizeof(T) == 4) {
+            if (R == 1) return launch_gather_inst<T, 1, uint32_t, COL, LZ>(m, A, st);
+        }
+        return HUBBARD_ERR_INVALID;      // dim >= 32767 only ever fits at 4 bytes per state
     }
     if constexpr (sizeof(T) == 4) {
-        if (R == 4) return launch_gather_vw<T, 4, uint16_t, COL, LZ>(m, A, st);
+        if (R == 4) return launch_gather_inst<T, 4, uint16_t, COL, LZ>(m, A, st);
     }
-    if (R >= 2) return launch_gather_vw<T, 2, uint16_t, COL, LZ>(m, A, st);
-    return launch_gather_vw<T, 1, uint16_t, COL, LZ>(m, A, st);
+    if (R >= 2) return launch_gather_inst<T, 2, uint16_t, COL, LZ>(m, A, st);
+    return launch_gather_inst<T, 1, uint16_t, COL, LZ>(m, A, st);
+}
+
+template <typename T>
+int launch_to_rt(hubbard_model *m, const T *x, T *rt, cudaStream_t st)
+{
+    const int R = gather_R(m);
+    const int64_t du = m->up.dim, dd = m->dn.dim, du_p = round_up(du, R), dd_p = round_up(dd, R);
+    const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((int64_t)m->sm_count * 8, (du_p / R * dd_p + 255) / 256));
+    if constexpr (sizeof(T) == 4) {
+        if (R == 4) { to_rt_kernel<T, 4><<<grid, 256, 0, st>>>(x, rt, du, dd, du_p, dd_p); return after_launch(m); }
+    }
+    if (R == 2) { to_rt_kernel<T, 2><<<grid, 256, 0, st>>>(x, rt, du, dd, du_p, dd_p); return after_launch(m); }
+    to_rt_kernel<T, 1><<<grid, 256, 0, st>>>(x, rt, du, dd, du_p, dd_p);
+    return after_launch(m);
+}
+
+int ensure_work(hubbard_model *m, int n_vec, size_t bytes)
+{
+    for (int i = 0; i < n_vec; ++i) {
+        if (m->work[i] && m->work_bytes[i] >= bytes) continue;
+        if (m->work[i]) cudaFree(m->work[i]);
+        m->work[i] = nullptr;
+        m->work_bytes[i] = 0;
+        CU_TRY(m, cudaMalloc(&m->work[i], std::max<size_t>(bytes, 16)));
+        m->work_bytes[i] = bytes;
+    }
+    return HUBBARD_OK;
 }
 
 // ---- variant PAPER
@@ -382,10 +410,13 @@ int apply_impl(hubbard_model *m, const T *x, T *y, cudaStream_t st)
     if (variant == HUBBARD_VARIANT_PAPER) return launch_paper<T, LZ>(m, x, y, st);
     if (variant == HUBBARD_VARIANT_GATHER) {
         if (LZ) return HUBBARD_ERR_INVALID;          // the Lanczos form of GATHER is lanczos_gather_impl
+        // two internal CT-layout vectors: x and z = (t H_dn + D) x
+        int rc = ensure_work(m, 2, (size_t)gather_vec_elems(m) * sizeof(T));
+        if (rc) return rc;
         GatherArgs<T> G{};
         G.x = x; G.y = y;
-        int rc = launch_gather<T, false, false>(m, G, st);
-        if (rc) return rc;
+        G.Wct = static_cast<T *>(m->work[0]); G.Zct = static_cast<T *>(m->work[1]);
+        if ((rc = launch_gather<T, false, false>(m, G, st))) return rc;
         return launch_gather<T, true, false>(m, G, st);
     }
     SweepArgs<T> A{x, y, LZ ? m->d_scal : nullptr, m->d_partial};
@@ -402,9 +433,9 @@ namespace {
 
 int ensure_lanczos_state(hubbard_model *m, int iters, int n_vec)
 {
-    const size_t bytes = (size_t)model_dim(m) * elem_size(m);
-    for (int i = 0; i < n_vec; ++i)
-        if (!m->work[i]) CU_TRY(m, cudaMalloc(&m->work[i], std::max<size_t>(bytes, 16)));
+    const size_t bytes = (size_t)(n_vec > 2 ? gather_vec_elems(m) : model_dim(m)) * elem_size(m);
+    int rc0 = ensure_work(m, n_vec, bytes);
+    if (rc0) return rc0;
     if (!m->d_scal) CU_TRY(m, cudaMalloc((void **)&m->d_scal, sizeof(LanczosScalars)));
     if (iters > m->coef_cap) {
         if (m->d_alpha) cudaFree(m->d_alpha);
@@ -433,36 +464,41 @@ int fetch_coefficients(hubbard_model *m, int iters, double *alpha, double *beta,
 }
 
 // Variant GATHER: two sweeps per iteration, vector updates folded in
-// (kernels_gather.cuh), one closing norm sweep for b_{m+1}.
+// (kernels_gather.cuh), one closing norm sweep for b_{m+1}.  Five work vectors:
+// A, B in the RT layout (q / u, swapped every iteration), two w buffers in the CT
+// layout (this iteration's w and the previous one = u_j) and z in CT.
 template <typename T>
 int lanczos_gather_impl(hubbard_model *m, const T *v0, int iters, double *alpha, double *beta, int *done,
                         cudaStream_t st)
 {
-    const int64_t dim = model_dim(m);
-    int rc = ensure_lanczos_state(m, iters, 3);
+    int rc = ensure_lanczos_state(m, iters, 5);
     if (rc) return rc;
-    const int vec_grid = (int)std::max<int64_t>(1, std::min<int64_t>((int64_t)m->sm_count * 4, (dim + 2047) / 2048));
+    const int64_t n_p = gather_vec_elems(m);
+    const int vec_grid = (int)std::max<int64_t>(1, std::min<int64_t>((int64_t)m->sm_count * 4, (n_p + 2047) / 2048));
     if ((rc = ensure_partials(m, std::max(vec_grid, m->sm_count)))) return rc;
-    T *Q = static_cast<T *>(m->work[0]), *F = static_cast<T *>(m->work[1]), *Z = static_cast<T *>(m->work[2]);
+    T *Art = static_cast<T *>(m->work[0]), *Brt = static_cast<T *>(m->work[1]);
+    T *wct[2] = {static_cast<T *>(m->work[2]), static_cast<T *>(m->work[3])};
+    T *zct = static_cast<T *>(m->work[4]);
     const double tau = m->tau >= 0 ? m->tau : (m->dtype == HUBBARD_F64 ? 1e-10 : 1e-5);
     {
         ProfScope ps(m, 5, st);
-        CU_TRY(m, cudaMemcpyAsync(Q, v0, (size_t)dim * sizeof(T), cudaMemcpyDeviceToDevice, st));   // "q_0" = f_1 unnormalised
-        CU_TRY(m, cudaMemsetAsync(F, 0, (size_t)dim * sizeof(T), st));                              // line 2: f_0 <- 0
+        if ((rc = launch_to_rt<T>(m, v0, Art, st))) return rc;                                      // "q_0" = f_1 unnormalised
+        CU_TRY(m, cudaMemsetAsync(Brt, 0, (size_t)n_p * sizeof(T), st));                            // line 2: f_0 <- 0
+        CU_TRY(m, cudaMemsetAsync(wct[1], 0, (size_t)n_p * sizeof(T), st));
         lanczos_scalars_init_kernel<<<1, 1, 0, st>>>(m->d_scal, tau);                               // line 1: b_1 <- 0
         if ((rc = after_launch(m))) return rc;
     }
     GatherArgs<T> G{};
-    G.S = m->d_scal; G.Z = Z; G.alpha_out = m->d_alpha; G.beta_out = m->d_beta;
+    G.S = m->d_scal; G.Zct = zct; G.alpha_out = m->d_alpha; G.beta_out = m->d_beta;
     for (int j = 0; j < iters; ++j) {
-        G.Q = Q; G.F = F;
+        G.Qrt = Art; G.Frt = Brt; G.Wct = wct[j & 1]; G.Fct = wct[(j + 1) & 1];
         if ((rc = launch_gather<T, false, true>(m, G, st))) return rc;     // lines 6-11 of j-1, row half of line 4
         if ((rc = launch_gather<T, true, true>(m, G, st))) return rc;      // line 4 (+ eq. 13), line 5
-        std::swap(Q, F);
+        std::swap(Art, Brt);
     }
     {
         ProfScope ps(m, 3, st);
-        lanczos_final_norm_kernel<T><<<vec_grid, 512, 0, st>>>(Q, F, dim, m->d_scal, m->d_partial, m->d_alpha, m->d_beta);
+        lanczos_final_norm_kernel<T><<<vec_grid, 512, 0, st>>>(Art, Brt, n_p, m->d_scal, m->d_partial, m->d_alpha, m->d_beta);
         if ((rc = after_launch(m))) return rc;
     }
     return fetch_coefficients(m, iters, alpha, beta, done, st);
@@ -550,7 +586,7 @@ void hubbard_destroy(hubbard_model *m)
     if (!m) return;
     for (auto &r : m->prof) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
     for (void *p : m->dev_allocs) cudaFree(p);
-    for (int i = 0; i < 3; ++i) if (m->work[i]) cudaFree(m->work[i]);
+    for (int i = 0; i < 5; ++i) if (m->work[i]) cudaFree(m->work[i]);
     for (int i = 0; i < 2; ++i) if (m->stage[i]) cudaFree(m->stage[i]);
     if (m->d_scal) cudaFree(m->d_scal);
     if (m->d_partial) cudaFree(m->d_partial);

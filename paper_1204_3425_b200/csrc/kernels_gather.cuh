@@ -16,14 +16,24 @@
 // [(kb * ld + i) * 8]) is read once per R outputs.  Padding entries point at a
 // zero slot.
 //
-// Lanczos form (Algorithm 1 with eq. 13), 8 vector passes per
-// iteration, no separate axpy/norm kernel:
-//   ROW sweep of iteration j+1:  w = q_j - a_j f_j  (line 6; staged AND written
-//        over q_j), b_{j+1}^2 = |w|^2 (line 7), z = (t H_dn + D) w  -> buffer Z;
-//        the last block records a_j, b_{j+1}, applies lines 8-10 and carries
-//        f_{j+1} = w / b_{j+1} (line 11) as the scalar c = 1/b_{j+1}.
+// Work vectors live in HBM in two TILE-MAJOR layouts, so that every tile either
+// sweep stages is ONE contiguous block that is already its shared-memory image
+// (du_p, dd_p = dim_up, dim_dn rounded up to R; padding holds zeros):
+//   RT  (row tiles)     element (a, b) at ((a / R) * dd_p + b) * R + a % R
+//   CT  (column tiles)  element (a, b) at ((b / R) * du_p + a) * R + b % R
+// A sweep reads its own layout contiguously and writes what the other sweep
+// will stage in the OTHER layout: the R x R block held by R adjacent lanes is
+// transposed with warp shuffles and each lane stores one 16-byte piece (full
+// 32/64-byte sectors, asynchronous) - all strided traffic is writes.
+//
+// Lanczos form (Algorithm 1 with eq. 13), no separate
+// axpy/norm kernel:
+//   ROW sweep of iteration j+1:  w = q_j - a_j f_j  (line 6; staged, written over
+//        q_j in RT and also in CT), b_{j+1}^2 = |w|^2 (line 7),
+//        z = (t H_dn + D) w -> CT; the last block records a_j, b_{j+1}, applies
+//        lines 8-10 and carries f_{j+1} = w / b_{j+1} (line 11) as c = 1/b_{j+1}.
 //   COL sweep of iteration j+1:  q_{j+1} = c (t H_up w + z) - b_{j+1} f_j  (line 4,
-//        written over f_j as in eq. 13) and a_{j+1} = q_{j+1} . f_{j+1} (line 5).
+//        written over f_j in RT as in eq. 13) and a_{j+1} = q_{j+1} . f_{j+1} (line 5).
 #pragma once
 #include "kernels_common.cuh"
 
@@ -36,13 +46,16 @@ template <typename T>
 struct GatherArgs {
     SpinDev in;             // the spin whose index is contracted (dn for ROW, up for COL)
     const uint32_t *st_out; // bit patterns of the other spin (ROW: states_up, for the diagonal)
-    int64_t dim_up, dim_dn;
+    int64_t dim_up, dim_dn; // du, dd
+    int64_t du_p, dd_p;     // rounded up to R
     double t, U;
-    // plain apply: y = H x
+    // plain apply: y = H x, both row-major (the ABI layout); xct, zct internal CT buffers
     const T *x;
     T *y;
-    // Lanczos: Q holds q_j -> w, F holds u_j (f_j = c_j u_j) -> q_{j+1}, Z the row-sweep result
-    T *Q, *F, *Z;
+    // Lanczos: Qrt holds q_j -> w, Frt holds u_j (f_j = c_j u_j) -> q_{j+1}   (RT layout)
+    //          Wct <- w, Zct <- z (written by ROW, read by COL), Fct = u_j      (CT layout)
+    T *Qrt, *Frt, *Wct, *Zct;
+    const T *Fct;
     LanczosScalars *S;
     double *partials;
     double *alpha_out, *beta_out;
@@ -119,27 +132,56 @@ __device__ __forceinline__ void lanczos_rotate(LanczosScalars *S, double b2, dou
     S->ticket = 0;
 }
 
+// ------------------------------------------------------------------ helpers
+template <typename T, int R>
+__device__ __forceinline__ T pick(const T (&v)[R], int idx)
+{
+    T r = v[0];
+#pragma unroll
+    for (int k = 1; k < R; ++k) r = (idx == k) ? v[k] : r;
+    return r;
+}
+
+// R adjacent lanes (q = lane % R) hold an R x R block, lane q holding column q
+// as v[r] = (row r, column q).  Returns in lane q the row q: o[c] = (row q, column c).
+template <typename T, int R>
+__device__ __forceinline__ Pack<T, R> block_transpose(const T (&v)[R], int q)
+{
+    Pack<T, R> o;
+    if (R == 1) {
+        o.v[0] = v[0];
+        return o;
+    }
+    T tmp[R];
+    tmp[0] = pick<T, R>(v, q);
+#pragma unroll
+    for (int d = 1; d < R; ++d) tmp[d] = __shfl_xor_sync(0xffffffffu, pick<T, R>(v, q ^ d), d);
+#pragma unroll
+    for (int c = 0; c < R; ++c) o.v[c] = pick<T, R>(tmp, c ^ q);
+    return o;
+}
+
 // ------------------------------------------------------------------ the sweep
-// T: storage/arithmetic type.  R: rows (ROW) or columns (COL) per tile.
-// E: hop entry type.  VW: elements per global vector access of the COL sweep
-// (divides R; needs dim_dn % VW == 0).  COL: which sweep.  LZ: Lanczos form.
-template <typename T, int R, typename E, int VW, bool COL, bool LZ>
+// T: storage/arithmetic type.  R: rows (ROW) and columns (COL) per tile.
+// E: hop entry type.  COL: which sweep.  LZ: Lanczos form.
+template <typename T, int R, typename E, bool COL, bool LZ>
 __global__ void __launch_bounds__(kGatherThreads, 1)
 gather_sweep_kernel(GatherArgs<T> A)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ double red[32];
     __shared__ int flag;
-    T *Xs = reinterpret_cast<T *>(smem_raw);              // [(n_in + 1)][R]
     using PR = Pack<T, R>;
-    using PV = Pack<T, VW>;
     using EB = Pack<E, kGatherBatch>;
+    PR *Xs = reinterpret_cast<PR *>(smem_raw);            // [n_in_p + 1]
     const unsigned char *xs_bytes = smem_raw;
 
     const int64_t dd = A.dim_dn, du = A.dim_up;
-    const int n_in = (int)A.in.dim;
-    const int64_t n_out = COL ? dd : du;
-    const int64_t n_tiles = (n_out + R - 1) / R;
+    const int n_in = (int)A.in.dim;                       // contracted dimension
+    const int n_in_p = (int)(COL ? A.du_p : A.dd_p);
+    const int n_in_w = (n_in_p + 31) & ~31;               // whole warps run the gather loop (shuffles)
+    const int64_t n_out_p = COL ? A.dd_p : A.du_p;
+    const int64_t n_tiles = n_out_p / R;
     const E *__restrict__ ent = ent_ptr<E>(A.in);
     const int64_t ld = A.in.ld;
     const T tt = (T)A.t, UU = (T)A.U;
@@ -154,54 +196,52 @@ gather_sweep_kernel(GatherArgs<T> A)
             bcp = (T)(A.S->beta * A.S->c_prev);           // b_{j+1} f_j = (b_{j+1} c_j) u_j
         }
     }
-    if (threadIdx.x < R) Xs[(int64_t)n_in * R + threadIdx.x] = T(0);     // the zero slot
+    if (threadIdx.x == 0) {
+        PR z;
+#pragma unroll
+        for (int r = 0; r < R; ++r) z.v[r] = T(0);
+        Xs[n_in_p] = z;                                   // the zero slot (== index n_in when n_in_p == n_in)
+    }
     double racc = 0.0;                                    // |w|^2 (ROW) or q.f (COL) partial
+    // buffers written in the other sweep's layout
+    PR *outW = reinterpret_cast<PR *>(A.Wct);             // ROW: w (or x) in CT
+    PR *outZ = reinterpret_cast<PR *>(COL ? A.Frt : A.Zct);   // ROW: z in CT;  COL/LZ: q in RT
 
     for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
         const int64_t o0 = tile * R;
-        const int nr = (int)min((int64_t)R, n_out - o0);
         __syncthreads();                                  // gathers of the previous tile are done
-        // ---- stage the tile, interleaved
-        if (!COL) {
+        // ---- stage the tile
+        if (COL || LZ) {
+            // tile-major layouts: the tile is one contiguous block, already interleaved
+            const PR *src = reinterpret_cast<const PR *>(COL ? A.Wct : A.Qrt) + tile * n_in_p;
+            if (!COL) {
+                const PR *fsrc = reinterpret_cast<const PR *>(A.Frt) + tile * n_in_p;
+                PR *wdst = reinterpret_cast<PR *>(A.Qrt) + tile * n_in_p;
+#pragma unroll 4
+                for (int i = threadIdx.x; i < n_in_p; i += kGatherThreads) {
+                    PR v = src[i];
+                    const PR f = fsrc[i];
 #pragma unroll
-            for (int r = 0; r < R; ++r) {
-                if (r < nr) {
-                    const int64_t J0 = (o0 + r) * dd;
-                    for (int b = threadIdx.x; b < n_in; b += kGatherThreads) {
-                        T v;
-                        if (LZ) {
-                            v = A.Q[J0 + b] - ac * A.F[J0 + b];
-                            A.Q[J0 + b] = v;
-                            racc += (double)v * (double)v;
-                        } else {
-                            v = A.x[J0 + b];
-                        }
-                        Xs[b * R + r] = v;
+                    for (int r = 0; r < R; ++r) {
+                        v.v[r] = v.v[r] - ac * f.v[r];
+                        racc += (double)v.v[r] * (double)v.v[r];
                     }
-                } else {
-                    for (int b = threadIdx.x; b < n_in; b += kGatherThreads) Xs[b * R + r] = T(0);
-                }
-            }
-        } else {
-            const T *src = LZ ? A.Q : A.x;
-            if (nr == R) {
-                for (int a = threadIdx.x; a < n_in; a += kGatherThreads) {
-                    const T *p = src + (int64_t)a * dd + o0;
-                    PR v;
-#pragma unroll
-                    for (int q = 0; q < R / VW; ++q) {
-                        PV u = *reinterpret_cast<const PV *>(p + q * VW);
-#pragma unroll
-                        for (int e = 0; e < VW; ++e) v.v[q * VW + e] = u.v[e];
-                    }
-                    *reinterpret_cast<PR *>(Xs + a * R) = v;
+                    wdst[i] = v;
+                    Xs[i] = v;
                 }
             } else {
-                for (int a = threadIdx.x; a < n_in; a += kGatherThreads) {
-                    const T *p = src + (int64_t)a * dd + o0;
+#pragma unroll 4
+                for (int i = threadIdx.x; i < n_in_p; i += kGatherThreads) Xs[i] = src[i];
+            }
+        } else {
+            // ROW sweep of hubbard_apply: x is the caller's row-major array
 #pragma unroll
-                    for (int r = 0; r < R; ++r) Xs[a * R + r] = (r < nr) ? p[r] : T(0);
-                }
+            for (int r = 0; r < R; ++r) {
+                const bool row_ok = o0 + r < du;
+                const T *xr = A.x + (o0 + r) * dd;
+                T *xs = reinterpret_cast<T *>(smem_raw) + r;
+                for (int b = threadIdx.x; b < n_in_p; b += kGatherThreads)
+                    xs[(int64_t)b * R] = (row_ok && b < n_in) ? xr[b] : T(0);
             }
         }
         __syncthreads();
@@ -210,10 +250,11 @@ gather_sweep_kernel(GatherArgs<T> A)
         uint32_t so[R];
         if (!COL) {
 #pragma unroll
-            for (int r = 0; r < R; ++r) so[r] = (r < nr) ? A.st_out[o0 + r] : 0u;
+            for (int r = 0; r < R; ++r) so[r] = (o0 + r < du) ? A.st_out[o0 + r] : 0u;
         }
-        for (int i = threadIdx.x; i < n_in; i += kGatherThreads) {
-            const int n = A.in.cnt[i];
+        for (int i = threadIdx.x; i < n_in_w; i += kGatherThreads) {
+            const bool valid = i < n_in;
+            const int n = valid ? A.in.cnt[i] : 0;
             T acc[R];
 #pragma unroll
             for (int r = 0; r < R; ++r) acc[r] = T(0);
@@ -233,54 +274,47 @@ gather_sweep_kernel(GatherArgs<T> A)
                 }
                 pk = nxt;
             }
-            const PR xi = *reinterpret_cast<const PR *>(Xs + i * R);
-            if (!COL) {
-                // Algorithm 4: on-the-fly diagonal; one write per element
-                const uint32_t sd = A.in.st[i];
+            const bool inpad = i < n_in_p;
+            PR xi;
 #pragma unroll
-                for (int r = 0; r < R; ++r) {
-                    if (r < nr) {
-                        const T h = tt * acc[r] + UU * (T)__popc(so[r] & sd) * xi.v[r];
-                        const int64_t J = (o0 + r) * dd + i;
-                        if (LZ) A.Z[J] = h; else A.y[J] = h;
-                    }
+            for (int r = 0; r < R; ++r) xi.v[r] = T(0);
+            if (inpad) xi = Xs[i];
+            const int q = i % R;
+            const int64_t oidx = (int64_t)(i / R) * n_out_p + o0 + q;    // this lane's 16-byte piece in the other layout
+            if (!COL) {
+                // Algorithm 4: on-the-fly diagonal
+                const uint32_t sd = valid ? A.in.st[i] : 0u;
+                T h[R];
+#pragma unroll
+                for (int r = 0; r < R; ++r) h[r] = tt * acc[r] + UU * (T)__popc(so[r] & sd) * xi.v[r];
+                const PR wt = block_transpose<T, R>(xi.v, q);
+                const PR zt = block_transpose<T, R>(h, q);
+                if (inpad) {
+                    outW[oidx] = wt;
+                    outZ[oidx] = zt;
                 }
             } else {
-                const int64_t J = (int64_t)i * dd + o0;
-                if (nr == R) {
+                PR z;
 #pragma unroll
-                    for (int q = 0; q < R / VW; ++q) {
-                        if (LZ) {
-                            PV f = *reinterpret_cast<const PV *>(A.F + J + q * VW);
-                            const PV z = *reinterpret_cast<const PV *>(A.Z + J + q * VW);
-#pragma unroll
-                            for (int e2 = 0; e2 < VW; ++e2) {
-                                const int r = q * VW + e2;
-                                const T qv = c * (tt * acc[r] + z.v[e2]) - bcp * f.v[e2];     // line 4 + eq. 13
-                                f.v[e2] = qv;
-                                racc += (double)qv * (double)(c * xi.v[r]);                     // line 5
-                            }
-                            *reinterpret_cast<PV *>(A.F + J + q * VW) = f;
-                        } else {
-                            PV yv = *reinterpret_cast<const PV *>(A.y + J + q * VW);
-#pragma unroll
-                            for (int e2 = 0; e2 < VW; ++e2) yv.v[e2] += tt * acc[q * VW + e2];
-                            *reinterpret_cast<PV *>(A.y + J + q * VW) = yv;
-                        }
-                    }
-                } else {
+                for (int r = 0; r < R; ++r) z.v[r] = T(0);
+                if (inpad) z = reinterpret_cast<const PR *>(A.Zct)[tile * n_in_p + i];
+                if (LZ) {
+                    PR f = z;
+                    if (inpad) f = reinterpret_cast<const PR *>(A.Fct)[tile * n_in_p + i];
+                    T qv[R];
 #pragma unroll
                     for (int r = 0; r < R; ++r) {
-                        if (r < nr) {
-                            if (LZ) {
-                                const T qv = c * (tt * acc[r] + A.Z[J + r]) - bcp * A.F[J + r];
-                                A.F[J + r] = qv;
-                                racc += (double)qv * (double)(c * xi.v[r]);
-                            } else {
-                                A.y[J + r] += tt * acc[r];
-                            }
-                        }
+                        qv[r] = c * (tt * acc[r] + z.v[r]) - bcp * f.v[r];      // line 4 + eq. 13
+                        racc += (double)qv[r] * (double)(c * xi.v[r]);          // line 5
                     }
+                    const PR qt = block_transpose<T, R>(qv, q);
+                    if (inpad) outZ[oidx] = qt;
+                } else if (valid) {
+                    // hubbard_apply: y is the caller's row-major array; one write per element
+                    T *yr = A.y + (int64_t)i * dd + o0;
+#pragma unroll
+                    for (int r = 0; r < R; ++r)
+                        if (o0 + r < dd) yr[r] = tt * acc[r] + z.v[r];
                 }
             }
         }
@@ -299,6 +333,26 @@ gather_sweep_kernel(GatherArgs<T> A)
                 }
             }
         }
+    }
+}
+
+// Start of a run: the caller's row-major start vector into the RT layout
+// (zero padding included).  One thread per 16-byte piece.
+template <typename T, int R>
+__global__ void __launch_bounds__(256)
+to_rt_kernel(const T *__restrict__ x, T *__restrict__ rt, int64_t du, int64_t dd, int64_t du_p, int64_t dd_p)
+{
+    using PR = Pack<T, R>;
+    const int64_t n = du_p / R * dd_p;
+    for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p < n; p += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t tile = p / dd_p, b = p - tile * dd_p;
+        PR v;
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int64_t a = tile * R + r;
+            v.v[r] = (a < du && b < dd) ? x[a * dd + b] : T(0);
+        }
+        reinterpret_cast<PR *>(rt)[p] = v;
     }
 }
 

@@ -85,7 +85,8 @@ struct hubbard_model {
     hub::DevModel dev{};
     std::vector<void *> dev_allocs;    // everything to cudaFree
     // Lanczos state (allocated on first use)
-    void *work[3] = {nullptr, nullptr, nullptr};   // third vector: variant GATHER only
+    void *work[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // 2 (PAPER/TWOSWEEP) or 5 (GATHER) in use
+    size_t work_bytes[5] = {0, 0, 0, 0, 0};
     hub::LanczosScalars *d_scal = nullptr;
     double *d_partial = nullptr;       // per-block partial sums
     int64_t n_partial = 0;
