@@ -14,7 +14,7 @@ from pathlib import Path
 PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libhubbard_b200.so"
-SOURCES = ["api.cu", "host_tables.cpp", "tridiag.cpp"]
+SOURCES = ["api.cu", "host_tables.cpp", "gather_tables.cpp", "tridiag.cpp"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
     "-Xcompiler", "-fPIC", "-shared", "-cudart", "static",

@@ -9,6 +9,7 @@
 #include "kernels_lanczos.cuh"
 #include "kernels_paper.cuh"
 #include "kernels_twosweep.cuh"
+#include "gather_tables.h"
 #include "model.h"
 
 using namespace hub;
@@ -66,32 +67,48 @@ int build_host(hubbard_model **out, int n_sites, int n_up, int n_dn, const int32
     return HUBBARD_OK;
 }
 
-// Column-major ELL of one spin for variant GATHER (kernels_gather.cuh).
-int upload_gather_table(hubbard_model *m, const SpinTable &tab, const uint32_t *d_states, SpinDev *out)
+int env_int(const char *name, int dflt)
+{
+    const char *v = getenv(name);
+    if (!v || !*v) return dflt;
+    return atoi(v);
+}
+
+// Tile height R (rows per ROW tile = columns per COL tile) of variant GATHER:
+// the largest R with R * sizeof(T) <= 16 for which a whole row AND a whole
+// column of V fit in shared memory; 0 if even R = 1 does not fit.
+int gather_R_for(const hubbard_model *m)
+{
+    const size_t es = m->dtype == HUBBARD_F32 ? 4 : 8;
+    const size_t budget = (size_t)std::max(0, m->max_smem_optin - 1024);
+    const int64_t n_in = std::max(m->dn.dim, m->up.dim);
+    int forced = env_int("HUBBARD_GATHER_R", 0);
+    for (int R = (int)(16 / es); R >= 1; R >>= 1) {
+        if (forced > 0 && R > forced) continue;
+        if ((size_t)(n_in + R + 128 / (R * es)) * R * es <= budget) return R;
+    }
+    return 0;
+}
+
+// Hop table of one spin for variant GATHER (kernels_gather.cuh, gather_tables.h).
+int upload_gather_table(hubbard_model *m, const SpinTable &tab, const uint32_t *d_states, int R, SpinDev *out)
 {
     SpinDev G{};
     G.dim = tab.dim;
-    G.w = (std::max(tab.width, 1) + 7) / 8 * 8;
-    G.ld = (tab.dim + 31) / 32 * 32;
     G.st = d_states;
-    const uint32_t pad = (uint32_t)tab.dim * 2u;
-    std::vector<uint32_t> e32((size_t)G.ld * G.w, pad);
-    std::vector<int32_t> cnt((size_t)tab.dim);
-    for (int64_t r = 0; r < tab.dim; ++r) {
-        int n = (int)(tab.rowptr[r + 1] - tab.rowptr[r]);
-        cnt[(size_t)r] = n;
-        for (int k = 0; k < n; ++k) {
-            size_t s = (size_t)(tab.rowptr[r] + k);
-            e32[((size_t)(k / 8) * G.ld + r) * 8 + k % 8] = (uint32_t)tab.col[s] * 2u + (tab.plus[s] ? 0u : 1u);
-        }
-    }
+    const int es = m->dtype == HUBBARD_F32 ? 4 : 8;
+    const int lanes = env_int("HUBBARD_GATHER_NOSCHED", 0) ? 0 : 128 / (R * es);
+    GatherTable T;
+    build_gather_table(tab, lanes, (tab.dim + R - 1) / R * R, T);
+    G.w = T.w;
+    G.ld = T.ld;
     int rc;
-    if ((rc = dev_upload(m, e32, &G.e32))) return rc;
-    if ((rc = dev_upload(m, cnt, &G.cnt))) return rc;
+    if ((rc = dev_upload(m, T.ent, &G.e32))) return rc;
+    if ((rc = dev_upload(m, T.cnt, &G.cnt))) return rc;
     G.e16 = nullptr;
-    if (tab.dim + 1 <= 32768) {
-        std::vector<uint16_t> e16(e32.size());
-        for (size_t i = 0; i < e32.size(); ++i) e16[i] = (uint16_t)e32[i];
+    if (tab.dim + 1 + 128 <= 32768) {
+        std::vector<uint16_t> e16(T.ent.size());
+        for (size_t i = 0; i < T.ent.size(); ++i) e16[i] = (uint16_t)T.ent[i];
         if ((rc = dev_upload(m, e16, &G.e16))) return rc;
     }
     *out = G;
@@ -144,8 +161,11 @@ int upload_tables(hubbard_model *m)
             if ((rc = dev_upload(m, d16, &D.dn_ent16))) return rc;
         }
         // variant GATHER: both spins column-major, entry = col * 2 + neg
-        if ((rc = upload_gather_table(m, m->up, D.st_up, &D.g_up))) return rc;
-        if ((rc = upload_gather_table(m, m->dn, D.st_dn, &D.g_dn))) return rc;
+        m->gather_R = gather_R_for(m);
+        if (m->gather_R > 0) {
+            if ((rc = upload_gather_table(m, m->up, D.st_up, m->gather_R, &D.g_up))) return rc;
+            if ((rc = upload_gather_table(m, m->dn, D.st_dn, m->gather_R, &D.g_dn))) return rc;
+        }
     } catch (const std::bad_alloc &) {
         return HUBBARD_ERR_HOST_OOM;
     }
@@ -188,13 +208,6 @@ int after_launch(hubbard_model *m)
     return HUBBARD_OK;
 }
 
-int env_int(const char *name, int dflt)
-{
-    const char *v = getenv(name);
-    if (!v || !*v) return dflt;
-    return atoi(v);
-}
-
 int ensure_partials(hubbard_model *m, int64_t n)
 {
     if (n <= m->n_partial) return HUBBARD_OK;
@@ -206,21 +219,7 @@ int ensure_partials(hubbard_model *m, int64_t n)
     return HUBBARD_OK;
 }
 
-// Tile height R (rows per ROW tile = columns per COL tile) of variant GATHER:
-// the largest R with R * sizeof(T) <= 16 for which a whole row AND a whole
-// column of V fit in shared memory; 0 if even R = 1 does not fit.
-int gather_R(const hubbard_model *m)
-{
-    const size_t es = m->dtype == HUBBARD_F32 ? 4 : 8;
-    const size_t budget = (size_t)std::max(0, m->max_smem_optin - 1024);
-    const int64_t n_in = std::max(m->dn.dim, m->up.dim);
-    int forced = env_int("HUBBARD_GATHER_R", 0);
-    for (int R = (int)(16 / es); R >= 1; R >>= 1) {
-        if (forced > 0 && R > forced) continue;
-        if ((size_t)(n_in + R + 1) * R * es <= budget) return R;
-    }
-    return 0;
-}
+int gather_R(const hubbard_model *m) { return m->gather_R; }
 
 bool gather_fits(const hubbard_model *m) { return gather_R(m) > 0; }
 
@@ -248,7 +247,7 @@ int launch_gather_inst(hubbard_model *m, GatherArgs<T> A, cudaStream_t st)
     A.du_p = round_up(A.dim_up, R);
     A.dd_p = round_up(A.dim_dn, R);
     const int64_t n_in_p = COL ? A.du_p : A.dd_p;
-    const size_t smem = (size_t)(n_in_p + 1) * R * sizeof(T);
+    const size_t smem = (size_t)(n_in_p + 128 / (R * sizeof(T))) * R * sizeof(T);
     CU_TRY(m, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const int64_t tiles = (COL ? A.dd_p : A.du_p) / R;
     const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(tiles, m->sm_count));

@@ -173,7 +173,8 @@ gather_sweep_kernel(GatherArgs<T> A)
     __shared__ int flag;
     using PR = Pack<T, R>;
     using EB = Pack<E, kGatherBatch>;
-    PR *Xs = reinterpret_cast<PR *>(smem_raw);            // [n_in_p + 1]
+    PR *Xs = reinterpret_cast<PR *>(smem_raw);            // [n_in_p + kZeroSlots]
+    constexpr int kZeroSlots = 128 / (int)sizeof(PR);     // lanes served by one shared-memory wavefront
     const unsigned char *xs_bytes = smem_raw;
 
     const int64_t dd = A.dim_dn, du = A.dim_up;
@@ -196,11 +197,11 @@ gather_sweep_kernel(GatherArgs<T> A)
             bcp = (T)(A.S->beta * A.S->c_prev);           // b_{j+1} f_j = (b_{j+1} c_j) u_j
         }
     }
-    if (threadIdx.x == 0) {
+    if (threadIdx.x < kZeroSlots) {
         PR z;
 #pragma unroll
         for (int r = 0; r < R; ++r) z.v[r] = T(0);
-        Xs[n_in_p] = z;                                   // the zero slot (== index n_in when n_in_p == n_in)
+        Xs[n_in_p + threadIdx.x] = z;                     // zero slots, one per bank group (padding entries)
     }
     double racc = 0.0;                                    // |w|^2 (ROW) or q.f (COL) partial
     // buffers written in the other sweep's layout
