@@ -247,12 +247,17 @@ int launch_gather_inst(hubbard_model *m, GatherArgs<T> A, cudaStream_t st)
     A.du_p = round_up(A.dim_up, R);
     A.dd_p = round_up(A.dim_dn, R);
     const int64_t n_in_p = COL ? A.du_p : A.dd_p;
-    const size_t smem = (size_t)(n_in_p + 128 / (R * sizeof(T))) * R * sizeof(T);
+    size_t smem = (size_t)(n_in_p + 128 / (R * sizeof(T))) * R * sizeof(T);
+    const size_t cnt_bytes = (size_t)round_up(n_in_p, 32);
+    A.cnt_in_smem = (A.in.w < 256 && smem + cnt_bytes + 1024 <= (size_t)m->max_smem_optin) ? 1 : 0;
+    if (A.cnt_in_smem) smem += cnt_bytes;
     CU_TRY(m, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const int64_t tiles = (COL ? A.dd_p : A.du_p) / R;
     const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(tiles, m->sm_count));
-    ProfScope ps(m, COL ? 2 : 1, st);
-    kern<<<grid, kGatherThreads, smem, st>>>(A);
+    {
+        ProfScope ps(m, COL ? 2 : 1, st);
+        kern<<<grid, kGatherThreads, smem, st>>>(A);
+    }
     return after_launch(m);
 }
 

@@ -39,8 +39,21 @@
 
 namespace hub {
 
-constexpr int kGatherThreads = 1024;
+#ifndef GS_THREADS
+#define GS_THREADS 1024
+#endif
+constexpr int kGatherThreads = GS_THREADS;
 constexpr int kGatherBatch = 8;          // hop entries fetched ahead per thread
+#ifndef GS_HOIST
+#define GS_HOIST 1
+#endif
+#ifndef GS_L2PF
+#define GS_L2PF 1
+#endif
+#ifndef GS_STAGE_UNROLL
+#define GS_STAGE_UNROLL 1
+#endif
+constexpr int kStageUnroll = GS_STAGE_UNROLL;          // 16-byte pieces in flight per thread while staging
 
 template <typename T>
 struct GatherArgs {
@@ -59,6 +72,7 @@ struct GatherArgs {
     LanczosScalars *S;
     double *partials;
     double *alpha_out, *beta_out;
+    int cnt_in_smem;        // hop counts cached in shared memory behind the tile (they fit and are < 256)
 };
 
 template <typename T, int N>
@@ -203,7 +217,13 @@ gather_sweep_kernel(GatherArgs<T> A)
         for (int r = 0; r < R; ++r) z.v[r] = T(0);
         Xs[n_in_p + threadIdx.x] = z;                     // zero slots, one per bank group (padding entries)
     }
+    unsigned char *cnt_s = smem_raw + (size_t)(n_in_p + kZeroSlots) * sizeof(PR);
+    if (A.cnt_in_smem)
+        for (int i = threadIdx.x; i < n_in_w; i += kGatherThreads) cnt_s[i] = (i < n_in) ? (unsigned char)A.in.cnt[i] : 0;
     double racc = 0.0;                                    // |w|^2 (ROW) or q.f (COL) partial
+    const int64_t tile_bytes = (int64_t)n_in_p * (int64_t)sizeof(PR);
+    const int n_it = (n_in_w + kGatherThreads - 1) / kGatherThreads;                // gather iterations per tile
+    const int64_t pf_slice = ((tile_bytes + n_it - 1) / n_it + 15) / 16 * 16;       // bytes of the next tile requested per iteration
     // buffers written in the other sweep's layout
     PR *outW = reinterpret_cast<PR *>(A.Wct);             // ROW: w (or x) in CT
     PR *outZ = reinterpret_cast<PR *>(COL ? A.Frt : A.Zct);   // ROW: z in CT;  COL/LZ: q in RT
@@ -218,21 +238,42 @@ gather_sweep_kernel(GatherArgs<T> A)
             if (!COL) {
                 const PR *fsrc = reinterpret_cast<const PR *>(A.Frt) + tile * n_in_p;
                 PR *wdst = reinterpret_cast<PR *>(A.Qrt) + tile * n_in_p;
-#pragma unroll 4
-                for (int i = threadIdx.x; i < n_in_p; i += kGatherThreads) {
-                    PR v = src[i];
-                    const PR f = fsrc[i];
+                // loads of kStageUnroll pieces are issued before the first store (w overwrites q in place)
+                for (int i0 = threadIdx.x; i0 < n_in_p; i0 += kStageUnroll * kGatherThreads) {
+                    PR v[kStageUnroll], f[kStageUnroll];
 #pragma unroll
-                    for (int r = 0; r < R; ++r) {
-                        v.v[r] = v.v[r] - ac * f.v[r];
-                        racc += (double)v.v[r] * (double)v.v[r];
+                    for (int u = 0; u < kStageUnroll; ++u) {
+                        const int i = i0 + u * kGatherThreads;
+                        if (i < n_in_p) { v[u] = src[i]; f[u] = fsrc[i]; }
                     }
-                    wdst[i] = v;
-                    Xs[i] = v;
+#pragma unroll
+                    for (int u = 0; u < kStageUnroll; ++u) {
+                        const int i = i0 + u * kGatherThreads;
+                        if (i < n_in_p) {
+#pragma unroll
+                            for (int r = 0; r < R; ++r) {
+                                v[u].v[r] = v[u].v[r] - ac * f[u].v[r];
+                                racc += (double)v[u].v[r] * (double)v[u].v[r];
+                            }
+                            wdst[i] = v[u];
+                            Xs[i] = v[u];
+                        }
+                    }
                 }
             } else {
-#pragma unroll 4
-                for (int i = threadIdx.x; i < n_in_p; i += kGatherThreads) Xs[i] = src[i];
+                for (int i0 = threadIdx.x; i0 < n_in_p; i0 += kStageUnroll * kGatherThreads) {
+                    PR v[kStageUnroll];
+#pragma unroll
+                    for (int u = 0; u < kStageUnroll; ++u) {
+                        const int i = i0 + u * kGatherThreads;
+                        if (i < n_in_p) v[u] = src[i];
+                    }
+#pragma unroll
+                    for (int u = 0; u < kStageUnroll; ++u) {
+                        const int i = i0 + u * kGatherThreads;
+                        if (i < n_in_p) Xs[i] = v[u];
+                    }
+                }
             }
         } else {
             // ROW sweep of hubbard_apply: x is the caller's row-major array
@@ -253,18 +294,53 @@ gather_sweep_kernel(GatherArgs<T> A)
 #pragma unroll
             for (int r = 0; r < R; ++r) so[r] = (o0 + r < du) ? A.st_out[o0 + r] : 0u;
         }
-        for (int i = threadIdx.x; i < n_in_w; i += kGatherThreads) {
+        int it = 0;
+        EB pk = load_batch(reinterpret_cast<const EB *>(ent) + threadIdx.x);    // every state has >= 1 (padding) batch
+        for (int i = threadIdx.x; i < n_in_w; i += kGatherThreads, ++it) {
             const bool valid = i < n_in;
-            const int n = valid ? A.in.cnt[i] : 0;
+            const bool inpad = i < n_in_p;
+            const int n = A.cnt_in_smem ? (int)cnt_s[i] : (valid ? A.in.cnt[i] : 0);
+            // operands of the epilogue: requested now, used after the gather
+            uint32_t sd = 0u;
+            PR z, f;
+#pragma unroll
+            for (int r = 0; r < R; ++r) z.v[r] = f.v[r] = T(0);
+#if GS_HOIST
+            if (!COL) {
+                if (valid) sd = A.in.st[i];
+            } else if (inpad) {
+                z = reinterpret_cast<const PR *>(A.Zct)[tile * n_in_p + i];
+                if (LZ) f = reinterpret_cast<const PR *>(A.Fct)[tile * n_in_p + i];
+            }
+#endif
+            // keep DRAM busy during the gather: a slice of the next tile's inputs goes to L2 every iteration
+#if GS_L2PF
+            if ((COL || LZ) && tile + gridDim.x < n_tiles) {
+                const int64_t off = (int64_t)it * pf_slice + (int64_t)threadIdx.x * 2048;
+                if (threadIdx.x * 2048 < pf_slice && off < tile_bytes) {
+                    const unsigned nb = (unsigned)min((int64_t)2048, min(pf_slice - (int64_t)threadIdx.x * 2048, tile_bytes - off));
+                    const char *p0 = reinterpret_cast<const char *>(reinterpret_cast<const PR *>(COL ? A.Wct : A.Qrt) +
+                                                                    (tile + gridDim.x) * n_in_p) + off;
+                    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p0), "r"(nb) : "memory");
+                    if (!COL) {
+                        const char *p1 = reinterpret_cast<const char *>(reinterpret_cast<const PR *>(A.Frt) +
+                                                                        (tile + gridDim.x) * n_in_p) + off;
+                        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p1), "r"(nb) : "memory");
+                    }
+                }
+            }
+#endif
             T acc[R];
 #pragma unroll
             for (int r = 0; r < R; ++r) acc[r] = T(0);
+            // one batch of hop entries is always in flight: the next batch of this state, or the first
+            // batch of this thread's next state (a state without hops still walks one padding batch)
             const EB *ep = reinterpret_cast<const EB *>(ent) + i;
-            EB pk = load_batch(ep);                       // every state has at least one (padding) batch
-            for (int k0 = 0; k0 < n; k0 += kGatherBatch) {
-                ep += ld;
-                EB nxt = pk;
-                if (k0 + kGatherBatch < n) nxt = load_batch(ep);        // fetch ahead: hides the L2 latency
+            const int nb = max(1, (n + kGatherBatch - 1) / kGatherBatch);
+            for (int b = 0; b < nb; ++b) {
+                const EB *np = (b + 1 < nb) ? ep + ld : reinterpret_cast<const EB *>(ent) + min(i + kGatherThreads, n_in_w - 1);
+                ep = np;
+                const EB nxt = load_batch(np);
 #pragma unroll
                 for (int j = 0; j < kGatherBatch; ++j) {
                     const uint32_t e = pk.v[j];
@@ -275,16 +351,22 @@ gather_sweep_kernel(GatherArgs<T> A)
                 }
                 pk = nxt;
             }
-            const bool inpad = i < n_in_p;
             PR xi;
 #pragma unroll
             for (int r = 0; r < R; ++r) xi.v[r] = T(0);
             if (inpad) xi = Xs[i];
+#if !GS_HOIST
+            if (!COL) {
+                if (valid) sd = A.in.st[i];
+            } else if (inpad) {
+                z = reinterpret_cast<const PR *>(A.Zct)[tile * n_in_p + i];
+                if (LZ) f = reinterpret_cast<const PR *>(A.Fct)[tile * n_in_p + i];
+            }
+#endif
             const int q = i % R;
             const int64_t oidx = (int64_t)(i / R) * n_out_p + o0 + q;    // this lane's 16-byte piece in the other layout
             if (!COL) {
                 // Algorithm 4: on-the-fly diagonal
-                const uint32_t sd = valid ? A.in.st[i] : 0u;
                 T h[R];
 #pragma unroll
                 for (int r = 0; r < R; ++r) h[r] = tt * acc[r] + UU * (T)__popc(so[r] & sd) * xi.v[r];
@@ -295,13 +377,7 @@ gather_sweep_kernel(GatherArgs<T> A)
                     outZ[oidx] = zt;
                 }
             } else {
-                PR z;
-#pragma unroll
-                for (int r = 0; r < R; ++r) z.v[r] = T(0);
-                if (inpad) z = reinterpret_cast<const PR *>(A.Zct)[tile * n_in_p + i];
                 if (LZ) {
-                    PR f = z;
-                    if (inpad) f = reinterpret_cast<const PR *>(A.Fct)[tile * n_in_p + i];
                     T qv[R];
 #pragma unroll
                     for (int r = 0; r < R; ++r) {
