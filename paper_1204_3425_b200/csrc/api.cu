@@ -236,7 +236,10 @@ int resolve_variant(const hubbard_model *m)
 {
     if (m->variant != HUBBARD_VARIANT_AUTO) return m->variant;
     if (m->dn.dim < 512 || m->up.dim < 512) return HUBBARD_VARIANT_PAPER;
-    return gather_fits(m) ? HUBBARD_VARIANT_GATHER : HUBBARD_VARIANT_TWOSWEEP;
+    // GATHER pays off when the R x R blocks it writes transposed are whole sectors (R * sizeof(T) = 16);
+    // with a narrower tile (C5 fp32: R = 1) its strided writes are 4-byte pieces and TWOSWEEP is faster.
+    const int es = m->dtype == HUBBARD_F32 ? 4 : 8;
+    return (gather_R(m) * es == 16) ? HUBBARD_VARIANT_GATHER : HUBBARD_VARIANT_TWOSWEEP;
 }
 
 // ---- variant GATHER

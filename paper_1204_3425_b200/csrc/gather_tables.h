@@ -8,7 +8,10 @@
 
 namespace hub {
 
-constexpr int kSlotBatch = 8;   // == kGatherBatch of the kernels
+#ifndef GS_BATCH
+#define GS_BATCH 8
+#endif
+constexpr int kSlotBatch = GS_BATCH;   // == kGatherBatch of the kernels
 
 struct GatherTable {
     int64_t ld = 0;                 // states per batch plane (dim rounded up to 32)

@@ -35,6 +35,7 @@
 //   COL sweep of iteration j+1:  q_{j+1} = c (t H_up w + z) - b_{j+1} f_j  (line 4,
 //        written over f_j in RT as in eq. 13) and a_{j+1} = q_{j+1} . f_{j+1} (line 5).
 #pragma once
+#include "gather_tables.h"
 #include "kernels_common.cuh"
 
 namespace hub {
@@ -43,7 +44,7 @@ namespace hub {
 #define GS_THREADS 1024
 #endif
 constexpr int kGatherThreads = GS_THREADS;
-constexpr int kGatherBatch = 8;          // hop entries fetched ahead per thread
+constexpr int kGatherBatch = kSlotBatch; // hop entries per batch (gather_tables.h), one batch always in flight
 #ifndef GS_HOIST
 #define GS_HOIST 1
 #endif
@@ -91,25 +92,23 @@ template <> __device__ __forceinline__ double sign_one<double>(uint32_t e)
     return __hiloint2double((int)(0x3ff00000u | (e << 31)), 0);
 }
 
-// One batch of kGatherBatch hop entries of one state: 16 (uint16) or 32 (uint32)
-// contiguous bytes, read through the read-only path.
-__device__ __forceinline__ Pack<uint16_t, 8> load_batch(const Pack<uint16_t, 8> *p)
+// One batch of kGatherBatch hop entries of one state: contiguous bytes, read
+// through the read-only path with the widest loads.
+template <typename E>
+__device__ __forceinline__ Pack<E, kGatherBatch> load_batch(const Pack<E, kGatherBatch> *p)
 {
-    const uint4 u = __ldg(reinterpret_cast<const uint4 *>(p));
-    Pack<uint16_t, 8> o;
-    o.v[0] = (uint16_t)(u.x & 0xffffu); o.v[1] = (uint16_t)(u.x >> 16);
-    o.v[2] = (uint16_t)(u.y & 0xffffu); o.v[3] = (uint16_t)(u.y >> 16);
-    o.v[4] = (uint16_t)(u.z & 0xffffu); o.v[5] = (uint16_t)(u.z >> 16);
-    o.v[6] = (uint16_t)(u.w & 0xffffu); o.v[7] = (uint16_t)(u.w >> 16);
-    return o;
-}
-__device__ __forceinline__ Pack<uint32_t, 8> load_batch(const Pack<uint32_t, 8> *p)
-{
-    const uint4 a = __ldg(reinterpret_cast<const uint4 *>(p));
-    const uint4 b = __ldg(reinterpret_cast<const uint4 *>(p) + 1);
-    Pack<uint32_t, 8> o;
-    o.v[0] = a.x; o.v[1] = a.y; o.v[2] = a.z; o.v[3] = a.w;
-    o.v[4] = b.x; o.v[5] = b.y; o.v[6] = b.z; o.v[7] = b.w;
+    constexpr int kBytes = (int)sizeof(E) * kGatherBatch;
+    Pack<E, kGatherBatch> o;
+    if constexpr (kBytes % 16 == 0) {
+        uint4 u[kBytes / 16];
+#pragma unroll
+        for (int k = 0; k < kBytes / 16; ++k) u[k] = __ldg(reinterpret_cast<const uint4 *>(p) + k);
+        memcpy(&o, u, kBytes);
+    } else {
+        static_assert(kBytes == 8, "batch must be 8 bytes or a multiple of 16");
+        const uint2 u = __ldg(reinterpret_cast<const uint2 *>(p));
+        memcpy(&o, &u, kBytes);
+    }
     return o;
 }
 

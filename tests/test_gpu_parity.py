@@ -82,6 +82,27 @@ def test_apply_vs_definition_small(ns, nu, nd, bonds, dtype, variant):
         assert rel_max_err(y, y_ref) <= TOL_HV[dtype]
 
 
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("R", [1, 2])
+def test_gather_narrow_tiles(R, dtype, monkeypatch):
+    """Variant GATHER with tile heights below the 16-byte width (what a large
+    sector would get: C5 fp32 has R = 1): H*v on C2 and a short Lanczos run,
+    forced through HUBBARD_GATHER_R (read by hubbard_create)."""
+    monkeypatch.setenv("HUBBARD_GATHER_R", str(R))
+    c = CONFIGS["C2"]
+    ref = RefModel(c.n_sites, c.n_up, c.n_dn, c.bonds, c.t, 4.0)
+    m = hb.hubbard_create(c.n_sites, c.n_up, c.n_dn, c.bonds, c.t, 4.0, dtype)
+    m.hubbard_set_variant(hb.VARIANT_GATHER)
+    x, x_np = start_vector(c.seed, c.dim, dtype)
+    y = torch.full_like(x, float("nan"))
+    m.hubbard_apply(x, y)
+    torch.cuda.synchronize()
+    assert rel_max_err(y, ref.apply(x_np)) <= TOL_HV[dtype]
+    alpha, beta = m.lanczos_run(x, 40)
+    a_ref, b_ref = lr.lanczos(ref.apply, x_np, 40)
+    assert abs(hb.lanczos_ground_energy(alpha, beta) - lr.ground_energy(a_ref, b_ref)) <= TOL_E0[dtype] * abs(lr.ground_energy(a_ref, b_ref))
+
+
 @pytest.mark.parametrize("variant", ["paper", "twosweep", "gather"])
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 @pytest.mark.parametrize("name", ["C1", "C2", "C3"])
