@@ -255,11 +255,17 @@ int launch_gather_inst(hubbard_model *m, GatherArgs<T> A, cudaStream_t st)
     A.cnt_in_smem = (A.in.w < 256 && smem + cnt_bytes + 1024 <= (size_t)m->max_smem_optin) ? 1 : 0;
     if (A.cnt_in_smem) smem += cnt_bytes;
     CU_TRY(m, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    CU_TRY(m, cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
     const int64_t tiles = (COL ? A.dd_p : A.du_p) / R;
-    const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(tiles, m->sm_count));
+    // Small sectors: several CTAs per SM (their staging and gather phases overlap one another); the 64-register
+    // kernels allow 1024 threads per SM in total.
+    int per_sm = (int)std::min<size_t>(4, (size_t)(m->max_smem_optin - 2048) / (smem + 1024));
+    per_sm = std::max(1, std::min(per_sm, env_int("HUBBARD_GATHER_CTAS", 4)));
+    const int threads = std::max(32, kGatherMaxThreads / per_sm / 32 * 32);
+    const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(tiles, (int64_t)m->sm_count * per_sm));
     {
         ProfScope ps(m, COL ? 2 : 1, st);
-        kern<<<grid, kGatherThreads, smem, st>>>(A);
+        kern<<<grid, threads, smem, st>>>(A);
     }
     return after_launch(m);
 }
@@ -273,7 +279,7 @@ int launch_gather(hubbard_model *m, GatherArgs<T> A, cudaStream_t st)
     A.dim_up = D.dim_up; A.dim_dn = D.dim_dn; A.t = m->t; A.U = m->U;
     const int R = gather_R(m);
     if (R == 0) return HUBBARD_ERR_INVALID;
-    if (LZ) { int rc = ensure_partials(m, m->sm_count); if (rc) return rc; A.partials = m->d_partial; }
+    if (LZ) { int rc = ensure_partials(m, (int64_t)m->sm_count * 4); if (rc) return rc; A.partials = m->d_partial; }
     if (!A.in.e16) {
         if constexpr (sizeof(T) == 4) {
             if (R == 1) return launch_gather_inst<T, 1, uint32_t, COL, LZ>(m, A, st);
@@ -482,7 +488,7 @@ int lanczos_gather_impl(hubbard_model *m, const T *v0, int iters, double *alpha,
     if (rc) return rc;
     const int64_t n_p = gather_vec_elems(m);
     const int vec_grid = (int)std::max<int64_t>(1, std::min<int64_t>((int64_t)m->sm_count * 4, (n_p + 2047) / 2048));
-    if ((rc = ensure_partials(m, std::max(vec_grid, m->sm_count)))) return rc;
+    if ((rc = ensure_partials(m, std::max<int64_t>(vec_grid, (int64_t)m->sm_count * 4)))) return rc;
     T *Art = static_cast<T *>(m->work[0]), *Brt = static_cast<T *>(m->work[1]);
     T *wct[2] = {static_cast<T *>(m->work[2]), static_cast<T *>(m->work[3])};
     T *zct = static_cast<T *>(m->work[4]);

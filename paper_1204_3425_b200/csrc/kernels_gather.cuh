@@ -40,10 +40,7 @@
 
 namespace hub {
 
-#ifndef GS_THREADS
-#define GS_THREADS 1024
-#endif
-constexpr int kGatherThreads = GS_THREADS;
+constexpr int kGatherMaxThreads = 1024;  // one CTA of 1024 threads per SM, or 2-4 smaller ones when their tiles fit together
 constexpr int kGatherBatch = kSlotBatch; // hop entries per batch (gather_tables.h), one batch always in flight
 #ifndef GS_HOIST
 #define GS_HOIST 1
@@ -178,7 +175,7 @@ __device__ __forceinline__ Pack<T, R> block_transpose(const T (&v)[R], int q)
 // T: storage/arithmetic type.  R: rows (ROW) and columns (COL) per tile.
 // E: hop entry type.  COL: which sweep.  LZ: Lanczos form.
 template <typename T, int R, typename E, bool COL, bool LZ>
-__global__ void __launch_bounds__(kGatherThreads, 1)
+__global__ void __launch_bounds__(kGatherMaxThreads, 1)
 gather_sweep_kernel(GatherArgs<T> A)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -190,6 +187,7 @@ gather_sweep_kernel(GatherArgs<T> A)
     constexpr int kZeroSlots = 128 / (int)sizeof(PR);     // lanes served by one shared-memory wavefront
     const unsigned char *xs_bytes = smem_raw;
 
+    const int nthr = (int)blockDim.x;                    // 1024, or less with several CTAs per SM (small sectors)
     const int64_t dd = A.dim_dn, du = A.dim_up;
     const int n_in = (int)A.in.dim;                       // contracted dimension
     const int n_in_p = (int)(COL ? A.du_p : A.dd_p);
@@ -218,10 +216,10 @@ gather_sweep_kernel(GatherArgs<T> A)
     }
     unsigned char *cnt_s = smem_raw + (size_t)(n_in_p + kZeroSlots) * sizeof(PR);
     if (A.cnt_in_smem)
-        for (int i = threadIdx.x; i < n_in_w; i += kGatherThreads) cnt_s[i] = (i < n_in) ? (unsigned char)A.in.cnt[i] : 0;
+        for (int i = threadIdx.x; i < n_in_w; i += nthr) cnt_s[i] = (i < n_in) ? (unsigned char)A.in.cnt[i] : 0;
     double racc = 0.0;                                    // |w|^2 (ROW) or q.f (COL) partial
     const int64_t tile_bytes = (int64_t)n_in_p * (int64_t)sizeof(PR);
-    const int n_it = (n_in_w + kGatherThreads - 1) / kGatherThreads;                // gather iterations per tile
+    const int n_it = (n_in_w + nthr - 1) / nthr;                // gather iterations per tile
     const int64_t pf_slice = ((tile_bytes + n_it - 1) / n_it + 15) / 16 * 16;       // bytes of the next tile requested per iteration
     // buffers written in the other sweep's layout
     PR *outW = reinterpret_cast<PR *>(A.Wct);             // ROW: w (or x) in CT
@@ -238,16 +236,16 @@ gather_sweep_kernel(GatherArgs<T> A)
                 const PR *fsrc = reinterpret_cast<const PR *>(A.Frt) + tile * n_in_p;
                 PR *wdst = reinterpret_cast<PR *>(A.Qrt) + tile * n_in_p;
                 // loads of kStageUnroll pieces are issued before the first store (w overwrites q in place)
-                for (int i0 = threadIdx.x; i0 < n_in_p; i0 += kStageUnroll * kGatherThreads) {
+                for (int i0 = threadIdx.x; i0 < n_in_p; i0 += kStageUnroll * nthr) {
                     PR v[kStageUnroll], f[kStageUnroll];
 #pragma unroll
                     for (int u = 0; u < kStageUnroll; ++u) {
-                        const int i = i0 + u * kGatherThreads;
+                        const int i = i0 + u * nthr;
                         if (i < n_in_p) { v[u] = src[i]; f[u] = fsrc[i]; }
                     }
 #pragma unroll
                     for (int u = 0; u < kStageUnroll; ++u) {
-                        const int i = i0 + u * kGatherThreads;
+                        const int i = i0 + u * nthr;
                         if (i < n_in_p) {
 #pragma unroll
                             for (int r = 0; r < R; ++r) {
@@ -260,16 +258,16 @@ gather_sweep_kernel(GatherArgs<T> A)
                     }
                 }
             } else {
-                for (int i0 = threadIdx.x; i0 < n_in_p; i0 += kStageUnroll * kGatherThreads) {
+                for (int i0 = threadIdx.x; i0 < n_in_p; i0 += kStageUnroll * nthr) {
                     PR v[kStageUnroll];
 #pragma unroll
                     for (int u = 0; u < kStageUnroll; ++u) {
-                        const int i = i0 + u * kGatherThreads;
+                        const int i = i0 + u * nthr;
                         if (i < n_in_p) v[u] = src[i];
                     }
 #pragma unroll
                     for (int u = 0; u < kStageUnroll; ++u) {
-                        const int i = i0 + u * kGatherThreads;
+                        const int i = i0 + u * nthr;
                         if (i < n_in_p) Xs[i] = v[u];
                     }
                 }
@@ -281,7 +279,7 @@ gather_sweep_kernel(GatherArgs<T> A)
                 const bool row_ok = o0 + r < du;
                 const T *xr = A.x + (o0 + r) * dd;
                 T *xs = reinterpret_cast<T *>(smem_raw) + r;
-                for (int b = threadIdx.x; b < n_in_p; b += kGatherThreads)
+                for (int b = threadIdx.x; b < n_in_p; b += nthr)
                     xs[(int64_t)b * R] = (row_ok && b < n_in) ? xr[b] : T(0);
             }
         }
@@ -295,7 +293,7 @@ gather_sweep_kernel(GatherArgs<T> A)
         }
         int it = 0;
         EB pk = load_batch(reinterpret_cast<const EB *>(ent) + threadIdx.x);    // every state has >= 1 (padding) batch
-        for (int i = threadIdx.x; i < n_in_w; i += kGatherThreads, ++it) {
+        for (int i = threadIdx.x; i < n_in_w; i += nthr, ++it) {
             const bool valid = i < n_in;
             const bool inpad = i < n_in_p;
             const int n = A.cnt_in_smem ? (int)cnt_s[i] : (valid ? A.in.cnt[i] : 0);
@@ -337,7 +335,7 @@ gather_sweep_kernel(GatherArgs<T> A)
             const EB *ep = reinterpret_cast<const EB *>(ent) + i;
             const int nb = max(1, (n + kGatherBatch - 1) / kGatherBatch);
             for (int b = 0; b < nb; ++b) {
-                const EB *np = (b + 1 < nb) ? ep + ld : reinterpret_cast<const EB *>(ent) + min(i + kGatherThreads, n_in_w - 1);
+                const EB *np = (b + 1 < nb) ? ep + ld : reinterpret_cast<const EB *>(ent) + min(i + nthr, n_in_w - 1);
                 ep = np;
                 const EB nxt = load_batch(np);
 #pragma unroll
