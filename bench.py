@@ -302,6 +302,23 @@ def run_native_dtype(args, cfg, U, dtype, rank, world, local):
     roof["fused_hv"]["achieved"] = roof["fused_hv"]["algorithmic_bytes"] / (hv_ms * 1e-3) / 1e9
     roof["fused_hv"]["frac"] = roof["fused_hv"]["achieved"] / peak
 
+    # ---- plain hubbard_apply (y = H x, caller's row-major vectors), for context: SURVEY 8(d) 2 x dim x s
+    y = torch.empty_like(v0)
+    for _ in range(3):
+        m.hubbard_apply(v0, y, stream)
+    a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    n_apply = 10
+    a0.record(stream)
+    for _ in range(n_apply):
+        m.hubbard_apply(v0, y, stream)
+    a1.record(stream)
+    torch.cuda.synchronize()
+    apply_ms = a0.elapsed_time(a1) / n_apply
+    apply = {"ms": apply_ms, "Hv_per_s": 1e3 / apply_ms, "algorithmic_bytes": 2 * cfg.dim * s,
+             "GBps": 2 * cfg.dim * s / (apply_ms * 1e-3) / 1e9}
+    apply["frac"] = apply["GBps"] / peak
+    del y
+
     # ---- end to end: host start vector (pinned) -> lanczos_run_host -> alpha/beta on the host
     e2e = None
     if not args.no_e2e:
@@ -325,7 +342,7 @@ def run_native_dtype(args, cfg, U, dtype, rank, world, local):
     return {
         "dtype": dtype, "value": world * args.steps * iters / (ms * 1e-3), "ms_per_step": ms / args.steps,
         "s_per_iteration": iter_ms * 1e-3, "roofline": roof, "kernels": kern, "e2e": e2e,
-        "gpu_launches": launches, "clocks": clk, "E0": e_0, "iters": iters,
+        "gpu_launches": launches, "clocks": clk, "E0": e_0, "iters": iters, "apply": apply,
     }
 
 
@@ -365,13 +382,14 @@ def main():
             "s_per_iteration": main_r["s_per_iteration"],
             "roofline": main_r["roofline"], "kernels": main_r["kernels"], "e2e": main_r["e2e"],
             "gpu_launches": main_r["gpu_launches"], "clocks": main_r["clocks"], "E0": main_r["E0"],
+            "hubbard_apply": main_r["apply"],
         }
         if cpu is not None:
             line["cpu_baseline"] = cpu
         for d in dtypes[1:]:
             r = results[d]
             line[d] = {k: r[k] for k in ("value", "ms_per_step", "s_per_iteration", "roofline", "kernels", "e2e",
-                                         "gpu_launches", "clocks", "E0")}
+                                         "gpu_launches", "clocks", "E0", "apply")}
         print(json.dumps(line))
     if world > 1:
         import torch.distributed as dist

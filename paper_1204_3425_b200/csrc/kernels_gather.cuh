@@ -70,6 +70,7 @@ struct GatherArgs {
     LanczosScalars *S;
     double *partials;
     double *alpha_out, *beta_out;
+    int y_rowmajor;         // ROW sweep of hubbard_apply writes y row-major (no CT buffers): hybrid with the strip sweep
     int cnt_in_smem;        // hop counts cached in shared memory behind the tile (they fit and are < 256)
 };
 
@@ -169,6 +170,31 @@ __device__ __forceinline__ Pack<T, R> block_transpose(const T (&v)[R], int q)
 #pragma unroll
     for (int c = 0; c < R; ++c) o.v[c] = pick<T, R>(tmp, c ^ q);
     return o;
+}
+
+// Stage R rows of a ROW-MAJOR vector interleaved: each thread loads VW consecutive columns of each of the R
+// rows (R vector loads in flight) and stores VW interleaved pieces.  n_in = dd must be a multiple of VW.
+template <typename T, int R, int VW>
+__device__ __forceinline__ void stage_rowmajor(const T *__restrict__ x, Pack<T, R> *Xs, int64_t o0, int64_t du, int64_t dd,
+                                               int n_in, int n_in_p, int nthr)
+{
+    using PV = Pack<T, VW>;
+    for (int b = (int)threadIdx.x * VW; b < n_in_p; b += nthr * VW) {
+        PV in[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+#pragma unroll
+            for (int c = 0; c < VW; ++c) in[r].v[c] = T(0);
+            if (o0 + r < du && b < n_in) in[r] = *reinterpret_cast<const PV *>(x + (o0 + r) * dd + b);
+        }
+#pragma unroll
+        for (int c = 0; c < VW; ++c) {
+            Pack<T, R> o;
+#pragma unroll
+            for (int r = 0; r < R; ++r) o.v[r] = in[r].v[c];
+            if (b + c < n_in_p) Xs[b + c] = o;
+        }
+    }
 }
 
 // ------------------------------------------------------------------ the sweep
@@ -274,14 +300,11 @@ gather_sweep_kernel(GatherArgs<T> A)
             }
         } else {
             // ROW sweep of hubbard_apply: x is the caller's row-major array
-#pragma unroll
-            for (int r = 0; r < R; ++r) {
-                const bool row_ok = o0 + r < du;
-                const T *xr = A.x + (o0 + r) * dd;
-                T *xs = reinterpret_cast<T *>(smem_raw) + r;
-                for (int b = threadIdx.x; b < n_in_p; b += nthr)
-                    xs[(int64_t)b * R] = (row_ok && b < n_in) ? xr[b] : T(0);
-            }
+            int vw = R;                                   // columns per vector load: rows must stay 16-byte aligned
+            while (vw > 1 && ((dd % vw) != 0 || (sizeof(T) * vw > 16))) vw >>= 1;
+            if (R >= 4 && vw == 4) stage_rowmajor<T, R, (R >= 4 ? 4 : 1)>(A.x, Xs, o0, du, dd, n_in, n_in_p, nthr);
+            else if (R >= 2 && vw >= 2) stage_rowmajor<T, R, (R >= 2 ? 2 : 1)>(A.x, Xs, o0, du, dd, n_in, n_in_p, nthr);
+            else stage_rowmajor<T, R, 1>(A.x, Xs, o0, du, dd, n_in, n_in_p, nthr);
         }
         __syncthreads();
 
@@ -367,11 +390,21 @@ gather_sweep_kernel(GatherArgs<T> A)
                 T h[R];
 #pragma unroll
                 for (int r = 0; r < R; ++r) h[r] = tt * acc[r] + UU * (T)__popc(so[r] & sd) * xi.v[r];
-                const PR wt = block_transpose<T, R>(xi.v, q);
-                const PR zt = block_transpose<T, R>(h, q);
-                if (inpad) {
-                    outW[oidx] = wt;
-                    outZ[oidx] = zt;
+                if (!LZ && A.y_rowmajor) {
+                    // hubbard_apply, hybrid form: y = (t H_dn + D) x in the caller's row-major layout
+                    // (coalesced over i for each of the R rows); the strip sweep adds the up term
+                    if (valid) {
+#pragma unroll
+                        for (int r = 0; r < R; ++r)
+                            if (o0 + r < du) A.y[(o0 + r) * dd + i] = h[r];
+                    }
+                } else {
+                    const PR wt = block_transpose<T, R>(xi.v, q);
+                    const PR zt = block_transpose<T, R>(h, q);
+                    if (inpad) {
+                        outW[oidx] = wt;
+                        outZ[oidx] = zt;
+                    }
                 }
             } else {
                 if (LZ) {
