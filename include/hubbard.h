@@ -167,6 +167,21 @@ int hubbard_get_basis(const hubbard_model *m, int spin, uint32_t *states_host);
 int hubbard_get_hops(const hubbard_model *m, int spin, int *width,
                      int32_t *cols_host, double *vals_host);
 
+/* hubbard_get_gather_table: the DEVICE layout of one spin's hop table as variant
+ * GATHER uses it (host computation only; works on hubbard_create_host models):
+ * the ELL format of PAPER.md:208-230 with batches of 8 entries of one state
+ * contiguous - entry k of state i at [((k / 8) * ld + i) * 8 + k % 8], entry =
+ * col * 2 + neg (element = t * (neg ? -1 : +1)) - and a state's
+ * entries placed in its slots so that the `lanes` lanes served by one
+ * shared-memory wavefront (8, 16 or 32; 0 = keep bond order) hit distinct banks.
+ * Padding entries have col >= zero_base (>= dim_spin: the zero slots of the
+ * staged tile).  Call first with entries_host == counts_host == NULL to obtain
+ * *slots (entries per state, a multiple of 8) and *ld; then pass
+ * entries_host[*ld * *slots] and counts_host[dim_spin] (last used slot + 1).
+ * *conflicts = entries that share a bank with another lane of their wavefront. */
+int hubbard_get_gather_table(const hubbard_model *m, int spin, int lanes, int64_t zero_base, int *slots, int64_t *ld,
+                             uint32_t *entries_host, int32_t *counts_host, int64_t *conflicts);
+
 /* ---- host utility, off the hot path ----
  * e0 = smallest eigenvalue of the symmetric tridiagonal T_m with diagonal
  * alpha[0..m-1] and off-diagonal beta[0..m-2]; m >= 1. */

@@ -20,7 +20,7 @@ KCLASS_NAMES = ("hv_paper", "row_sweep", "col_sweep", "vec_sweep", "scalar", "se
 ABI_SYMBOLS = (
     "hubbard_create", "hubbard_create_host", "hubbard_destroy", "hubbard_dims", "hubbard_set_U",
     "hubbard_set_variant", "hubbard_apply", "lanczos_run", "lanczos_set_tau", "hubbard_apply_host",
-    "lanczos_run_host", "hubbard_get_basis", "hubbard_get_hops", "lanczos_ground_energy",
+    "lanczos_run_host", "hubbard_get_basis", "hubbard_get_hops", "hubbard_get_gather_table", "lanczos_ground_energy",
     "hubbard_profile", "hubbard_kernel_times", "hubbard_launch_count", "hubbard_last_cuda_error",
     "hubbard_strerror",
 )
@@ -28,8 +28,11 @@ ABI_SYMBOLS = (
 
 def _load() -> C.CDLL:
     path: Path = _build.LIB
-    if not path.exists():
-        path = _build.build()
+    try:
+        path = _build.build()            # no-op when the library is newer than its sources
+    except Exception:
+        if not path.exists():            # no usable library and no compiler: there is no fallback
+            raise
     lib = C.CDLL(str(path))
     vp, i32, i64, dbl = C.c_void_p, C.c_int, C.c_int64, C.c_double
     P = C.POINTER
@@ -47,6 +50,7 @@ def _load() -> C.CDLL:
     lib.lanczos_run_host.argtypes = [vp, vp, i32, P(dbl), P(dbl), P(i32), vp]
     lib.hubbard_get_basis.argtypes = [vp, i32, P(C.c_uint32)]
     lib.hubbard_get_hops.argtypes = [vp, i32, P(i32), P(C.c_int32), P(dbl)]
+    lib.hubbard_get_gather_table.argtypes = [vp, i32, i32, i64, P(i32), P(i64), P(C.c_uint32), P(C.c_int32), P(i64)]
     lib.lanczos_ground_energy.argtypes = [P(dbl), P(dbl), i32, P(dbl)]
     lib.hubbard_profile.argtypes = [vp, i32]
     lib.hubbard_kernel_times.argtypes = [vp, P(i64), P(dbl)]
@@ -197,6 +201,20 @@ class Model:
         _check(lib.hubbard_get_hops(self._h, spin, C.byref(w), cols.ctypes.data_as(C.POINTER(C.c_int32)),
                                     vals.ctypes.data_as(C.POINTER(C.c_double))), "hubbard_get_hops")
         return w.value, cols, vals
+
+    def hubbard_get_gather_table(self, spin, lanes, zero_base=None):
+        """(slots, ld, entries[slots/8, ld, 8], counts[dim_spin], conflicts) of variant GATHER's table."""
+        n = self.dim_up if spin == 0 else self.dim_dn
+        zb = n if zero_base is None else int(zero_base)
+        w, ld, cf = C.c_int(0), C.c_int64(0), C.c_int64(0)
+        _check(lib.hubbard_get_gather_table(self._h, spin, lanes, zb, C.byref(w), C.byref(ld), None, None, C.byref(cf)),
+               "hubbard_get_gather_table")
+        ent = np.empty((w.value // 8, ld.value, 8), dtype=np.uint32)
+        cnt = np.empty(n, dtype=np.int32)
+        _check(lib.hubbard_get_gather_table(self._h, spin, lanes, zb, C.byref(w), C.byref(ld),
+                                            ent.ctypes.data_as(C.POINTER(C.c_uint32)),
+                                            cnt.ctypes.data_as(C.POINTER(C.c_int32)), C.byref(cf)), "hubbard_get_gather_table")
+        return w.value, ld.value, ent, cnt, cf.value
 
     # -- measurement hooks
     def hubbard_profile(self, enable=True):

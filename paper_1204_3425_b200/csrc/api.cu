@@ -724,6 +724,26 @@ int hubbard_get_hops(const hubbard_model *m, int spin, int *width, int32_t *cols
     return HUBBARD_OK;
 }
 
+int hubbard_get_gather_table(const hubbard_model *m, int spin, int lanes, int64_t zero_base, int *slots, int64_t *ld,
+                             uint32_t *entries_host, int32_t *counts_host, int64_t *conflicts)
+{
+    if (!m || (spin != 0 && spin != 1) || lanes < 0 || lanes > 32 || (lanes & (lanes - 1)) != 0) return HUBBARD_ERR_INVALID;
+    const SpinTable &tab = spin == 0 ? m->up : m->dn;
+    if (zero_base < tab.dim) return HUBBARD_ERR_INVALID;
+    try {
+        GatherTable T;
+        build_gather_table(tab, lanes, zero_base, T);
+        if (slots) *slots = T.w;
+        if (ld) *ld = T.ld;
+        if (conflicts) *conflicts = T.conflicts;
+        if (entries_host) std::memcpy(entries_host, T.ent.data(), T.ent.size() * sizeof(uint32_t));
+        if (counts_host) std::memcpy(counts_host, T.cnt.data(), T.cnt.size() * sizeof(int32_t));
+    } catch (const std::bad_alloc &) {
+        return HUBBARD_ERR_HOST_OOM;
+    }
+    return HUBBARD_OK;
+}
+
 int hubbard_profile(hubbard_model *m, int enable)
 {
     if (!m) return HUBBARD_ERR_INVALID;

@@ -149,3 +149,48 @@ def test_ground_energy_vs_lapack():
     assert hb.lanczos_ground_energy([3.0, -1.0, 2.0], [0.0, 0.0], 1) == pytest.approx(3.0, abs=1e-14)
     with pytest.raises(hb.HubbardError):
         hb.lanczos_ground_energy([float("nan")], [0.0], 1)
+
+
+@pytest.mark.parametrize("lanes", [0, 8, 16, 32])
+@pytest.mark.parametrize("name,ns,nu,nd,bonds", [
+    ("C4", 16, 8, 8, torus_bonds(4, 4)), ("C2", 12, 6, 6, ring_bonds(12)), ("odd", 7, 3, 4, ring_bonds(7) + [(0, 3), (2, 6)]),
+    ("dup", 6, 3, 3, ring_bonds(6) + [(0, 1)])])
+def test_gather_table_is_a_bank_aware_permutation_of_the_hops(name, ns, nu, nd, bonds, lanes):
+    """The device table of variant GATHER (host computation): per state the same
+    multiset of (column, sign) as the canonical hop list (duplicates kept as
+    separate entries), padding only beyond the sector, counts cover every real
+    entry, and - with scheduling on - (almost) no two lanes of a shared-memory
+    wavefront on one bank."""
+    m = hb.hubbard_create_host(ns, nu, nd, bonds, 1.0, 0.0)
+    ref = RefModel(ns, nu, nd, bonds, 1.0, 0.0)
+    for spin in (0, 1):
+        n = m.dim_up if spin == 0 else m.dim_dn
+        zero_base = (n + 1) // 2 * 2
+        w, ld, ent, cnt, conflicts = m.hubbard_get_gather_table(spin, lanes, zero_base)
+        assert w % 8 == 0 and ld % 32 == 0 and ld >= n
+        flat = ent.transpose(1, 0, 2).reshape(ld, w)            # [state][slot]
+        rows = ref.hop_rows(spin)
+        n_real = 0
+        for i in range(n):
+            e = flat[i, :cnt[i]]
+            real = e[(e >> 1) < n]
+            assert np.all((flat[i, cnt[i]:] >> 1) >= zero_base)                 # beyond the count: padding only
+            assert np.all((e[(e >> 1) >= n] >> 1) >= zero_base)
+            got = {}
+            for x in real:                                                      # merge duplicates like the canonical form
+                got[int(x >> 1)] = got.get(int(x >> 1), 0.0) + (-1.0 if x & 1 else 1.0)
+            assert {c: v for c, v in got.items() if v != 0.0} == {c: v for c, v in rows[i]}
+            n_real += len(real)
+        if lanes:
+            # wavefront groups of `lanes` consecutive states: distinct banks per slot, up to the reported conflicts
+            worst = 0
+            for g0 in range(0, n, lanes):
+                blk = flat[g0:min(n, g0 + lanes)]
+                for s in range(w):
+                    col = blk[:, s] >> 1
+                    used = col[np.arange(len(blk)) + g0 < n]
+                    used = used[[s < cnt[g0 + k] for k in range(len(used))]]
+                    banks = used % lanes
+                    worst += len(banks) - len(np.unique(banks))
+            assert worst <= conflicts
+            assert conflicts <= max(4, n_real // 200)
