@@ -319,6 +319,24 @@ def run_native_dtype(args, cfg, U, dtype, rank, world, local):
     apply["frac"] = apply["GBps"] / peak
     del y
 
+    # ---- SURVEY 8(f)-2 (measured once, outside the headline): convergence-driven stop and the ground-state vector
+    nxt = None
+    if dtype == "f64" and not args.no_e2e:
+        t0 = time.perf_counter()
+        a_u, b_u, e_u = m.lanczos_run_until(v0, iters, 10, 1e-12, stream)
+        t_until = time.perf_counter() - t0
+        psi = torch.empty_like(v0)
+        t0 = time.perf_counter()
+        e_gs, n_gs = m.lanczos_ground_state(v0, iters, psi, stream)
+        t_gs = time.perf_counter() - t0
+        hp = torch.empty_like(psi)
+        m.hubbard_apply(psi, hp, stream)
+        torch.cuda.synchronize()
+        resid = float((hp - e_gs * psi).abs().max().item())
+        nxt = {"run_until": {"tol": 1e-12, "check_every": 10, "iters_done": len(a_u), "E0": e_u, "s": t_until},
+               "ground_state": {"iters": n_gs, "E0": e_gs, "s": t_gs, "max_abs_residual": resid}}
+        del psi, hp
+
     # ---- end to end: host start vector (pinned) -> lanczos_run_host -> alpha/beta on the host
     e2e = None
     if not args.no_e2e:
@@ -342,7 +360,7 @@ def run_native_dtype(args, cfg, U, dtype, rank, world, local):
     return {
         "dtype": dtype, "value": world * args.steps * iters / (ms * 1e-3), "ms_per_step": ms / args.steps,
         "s_per_iteration": iter_ms * 1e-3, "roofline": roof, "kernels": kern, "e2e": e2e,
-        "gpu_launches": launches, "clocks": clk, "E0": e_0, "iters": iters, "apply": apply,
+        "gpu_launches": launches, "clocks": clk, "E0": e_0, "iters": iters, "apply": apply, "next": nxt,
     }
 
 
@@ -382,7 +400,7 @@ def main():
             "s_per_iteration": main_r["s_per_iteration"],
             "roofline": main_r["roofline"], "kernels": main_r["kernels"], "e2e": main_r["e2e"],
             "gpu_launches": main_r["gpu_launches"], "clocks": main_r["clocks"], "E0": main_r["E0"],
-            "hubbard_apply": main_r["apply"],
+            "hubbard_apply": main_r["apply"], "next_rows": main_r["next"],
         }
         if cpu is not None:
             line["cpu_baseline"] = cpu

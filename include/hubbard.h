@@ -139,6 +139,30 @@ int hubbard_apply(hubbard_model *m, const void *x_dev, void *y_dev, void *stream
 int lanczos_run(hubbard_model *m, const void *v0_dev, int iters,
                 double *alpha_host, double *beta_host, int *iters_done, void *stream);
 
+/* lanczos_run_until: lanczos_run with the convergence check of PAPER.md:146
+ * ("the convergence of the ground state energy can be checked after each
+ * iteration").  Every `check_every` iterations (>= 1) the coefficients so far
+ * are brought to the host, E_0^(m) = lambda_min(T_m) is computed and the run
+ * stops when |E_0^(m) - E_0^(m - check_every)| <= tol * max(1, |E_0^(m)|), on
+ * breakdown, or after max_iters iterations.  alpha_host / beta_host (max_iters
+ * doubles each) and iters_done are as in lanczos_run; *e0 (may be NULL) =
+ * lambda_min(T_m) for m = iters_done.  Each check synchronises the stream. */
+int lanczos_run_until(hubbard_model *m, const void *v0_dev, int max_iters, int check_every, double tol,
+                      double *alpha_host, double *beta_host, int *iters_done, double *e0, void *stream);
+
+/* lanczos_ground_state: the approximate ground-state VECTOR after `iters`
+ * Lanczos iterations.  The two-vector scheme discards the Lanczos basis
+ * (PAPER.md:154), so the run is done twice: pass 1 gives T_m, the host computes
+ * its lowest eigenvector y, pass 2 repeats the identical run
+ * (all reductions are deterministic) and accumulates psi = sum_j y_j f_j.
+ *   psi_dev  device, dim elements of the model's dtype, row-major (element
+ *            J = i_up*dim_dn + i_dn), caller-owned, 16-byte aligned, != v0_dev;
+ *            normalised to |psi| = 1 on return.
+ *   e0       may be NULL: lambda_min(T_m), m = *iters_done (< iters on breakdown)
+ * Synchronises the stream before returning. */
+int lanczos_ground_state(hubbard_model *m, const void *v0_dev, int iters, void *psi_dev, double *e0, int *iters_done,
+                         void *stream);
+
 /* Breakdown threshold tau (>= 0; 0 = the paper's literal "b = 0" test). */
 int lanczos_set_tau(hubbard_model *m, double tau);
 
@@ -186,6 +210,8 @@ int hubbard_get_gather_table(const hubbard_model *m, int spin, int lanes, int64_
  * e0 = smallest eigenvalue of the symmetric tridiagonal T_m with diagonal
  * alpha[0..m-1] and off-diagonal beta[0..m-2]; m >= 1. */
 int lanczos_ground_energy(const double *alpha, const double *beta, int m, double *e0);
+/* Same, plus the eigenvector y (m doubles, unit norm, y[0] >= 0) of that eigenvalue (inverse iteration); e0 may be NULL. */
+int lanczos_ground_vector(const double *alpha, const double *beta, int m, double *e0, double *y);
 
 /* ---- measurement hooks ----
  * hubbard_profile(m, 1) makes every later kernel launch of this model be

@@ -19,7 +19,8 @@ KCLASS_NAMES = ("hv_paper", "row_sweep", "col_sweep", "vec_sweep", "scalar", "se
 
 ABI_SYMBOLS = (
     "hubbard_create", "hubbard_create_host", "hubbard_destroy", "hubbard_dims", "hubbard_set_U",
-    "hubbard_set_variant", "hubbard_apply", "lanczos_run", "lanczos_set_tau", "hubbard_apply_host",
+    "hubbard_set_variant", "hubbard_apply", "lanczos_run", "lanczos_run_until", "lanczos_ground_state",
+    "lanczos_ground_vector", "lanczos_set_tau", "hubbard_apply_host",
     "lanczos_run_host", "hubbard_get_basis", "hubbard_get_hops", "hubbard_get_gather_table", "lanczos_ground_energy",
     "hubbard_profile", "hubbard_kernel_times", "hubbard_launch_count", "hubbard_last_cuda_error",
     "hubbard_strerror",
@@ -46,6 +47,9 @@ def _load() -> C.CDLL:
     lib.hubbard_apply.argtypes = [vp, vp, vp, vp]
     lib.lanczos_run.argtypes = [vp, vp, i32, P(dbl), P(dbl), P(i32), vp]
     lib.lanczos_set_tau.argtypes = [vp, dbl]
+    lib.lanczos_run_until.argtypes = [vp, vp, i32, i32, dbl, P(dbl), P(dbl), P(i32), P(dbl), vp]
+    lib.lanczos_ground_state.argtypes = [vp, vp, i32, vp, P(dbl), P(i32), vp]
+    lib.lanczos_ground_vector.argtypes = [P(dbl), P(dbl), i32, P(dbl), P(dbl)]
     lib.hubbard_apply_host.argtypes = [vp, vp, vp, vp]
     lib.lanczos_run_host.argtypes = [vp, vp, i32, P(dbl), P(dbl), P(i32), vp]
     lib.hubbard_get_basis.argtypes = [vp, i32, P(C.c_uint32)]
@@ -161,6 +165,24 @@ class Model:
                                C.byref(done), _stream(stream)), "lanczos_run", self._h)
         return alpha[:done.value].copy(), beta[:done.value].copy()
 
+    def lanczos_run_until(self, v0, max_iters, check_every=10, tol=1e-12, stream=None):
+        """(alpha, beta, e0): stops when E_0 moved by <= tol * max(1, |E_0|) over `check_every` iterations."""
+        alpha = np.zeros(max(max_iters, 1))
+        beta = np.zeros(max(max_iters, 1))
+        done, e0 = C.c_int(0), C.c_double(0.0)
+        dp = C.POINTER(C.c_double)
+        _check(lib.lanczos_run_until(self._h, _dptr(v0), max_iters, check_every, float(tol), alpha.ctypes.data_as(dp),
+                                     beta.ctypes.data_as(dp), C.byref(done), C.byref(e0), _stream(stream)),
+               "lanczos_run_until", self._h)
+        return alpha[:done.value].copy(), beta[:done.value].copy(), e0.value
+
+    def lanczos_ground_state(self, v0, iters, psi, stream=None):
+        """Fills psi (device tensor, dim elements) with the normalised ground-state vector; returns (e0, iters_done)."""
+        done, e0 = C.c_int(0), C.c_double(0.0)
+        _check(lib.lanczos_ground_state(self._h, _dptr(v0), iters, _dptr(psi), C.byref(e0), C.byref(done), _stream(stream)),
+               "lanczos_ground_state", self._h)
+        return e0.value, done.value
+
     # -- hot path, host buffers (numpy arrays or CPU torch tensors)
     @staticmethod
     def _hptr(a) -> int:
@@ -251,3 +273,20 @@ def lanczos_ground_energy(alpha, beta, m=None) -> float:
     _check(lib.lanczos_ground_energy(a.ctypes.data_as(dp), b.ctypes.data_as(dp), m, C.byref(e0)),
            "lanczos_ground_energy")
     return e0.value
+
+
+def lanczos_ground_vector(alpha, beta, m=None):
+    """(e0, y): smallest eigenvalue of T_m and its unit eigenvector (host utility)."""
+    a = np.ascontiguousarray(alpha, dtype=np.float64)
+    b = np.ascontiguousarray(beta, dtype=np.float64)
+    m = len(a) if m is None else int(m)
+    if len(b) < max(m - 1, 0) or len(a) < m:
+        raise ValueError("alpha/beta shorter than m")
+    if len(b) == 0:
+        b = np.zeros(1)
+    e0 = C.c_double(0.0)
+    y = np.zeros(m)
+    dp = C.POINTER(C.c_double)
+    _check(lib.lanczos_ground_vector(a.ctypes.data_as(dp), b.ctypes.data_as(dp), m, C.byref(e0), y.ctypes.data_as(dp)),
+           "lanczos_ground_vector")
+    return e0.value, y

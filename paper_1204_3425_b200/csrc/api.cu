@@ -307,6 +307,20 @@ int launch_to_rt(hubbard_model *m, const T *x, T *rt, cudaStream_t st)
     return after_launch(m);
 }
 
+template <typename T>
+int launch_from_rt(hubbard_model *m, const T *rt, T *x, cudaStream_t st)
+{
+    const int R = gather_R(m);
+    const int64_t du = m->up.dim, dd = m->dn.dim, du_p = round_up(du, R), dd_p = round_up(dd, R);
+    const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((int64_t)m->sm_count * 8, (du_p / R * dd_p + 255) / 256));
+    if constexpr (sizeof(T) == 4) {
+        if (R == 4) { from_rt_kernel<T, 4><<<grid, 256, 0, st>>>(rt, x, du, dd, du_p, dd_p); return after_launch(m); }
+    }
+    if (R == 2) { from_rt_kernel<T, 2><<<grid, 256, 0, st>>>(rt, x, du, dd, du_p, dd_p); return after_launch(m); }
+    from_rt_kernel<T, 1><<<grid, 256, 0, st>>>(rt, x, du, dd, du_p, dd_p);
+    return after_launch(m);
+}
+
 int ensure_work(hubbard_model *m, int n_vec, size_t bytes)
 {
     for (int i = 0; i < n_vec; ++i) {
@@ -487,67 +501,91 @@ int fetch_coefficients(hubbard_model *m, int iters, double *alpha, double *beta,
     return HUBBARD_OK;
 }
 
+// What one call of the Lanczos engine does: iterations [j0, j1) of Algorithm 1,
+// optionally the start (copy of v0, scalars) and the closing norm; with `ycoef`
+// it also accumulates psi += y_j f_j (second pass for the ground-state vector).
+struct LanczosPlan {
+    int j0 = 0, j1 = 0;
+    bool init = true, finish = true;
+    const double *ycoef = nullptr;   // device, y_1..y_m of T_m's eigenvector
+    void *psi = nullptr;             // device, same layout as the engine's vectors
+};
+
+int lanczos_vec_grid(const hubbard_model *m, int64_t n)
+{
+    return (int)std::max<int64_t>(1, std::min<int64_t>((int64_t)m->sm_count * 4, (n + 2047) / 2048));
+}
+
+double lanczos_tau(const hubbard_model *m) { return m->tau >= 0 ? m->tau : (m->dtype == HUBBARD_F64 ? 1e-10 : 1e-5); }
+
 // Variant GATHER: two sweeps per iteration, vector updates folded in
 // (kernels_gather.cuh), one closing norm sweep for b_{m+1}.  Five work vectors:
 // A, B in the RT layout (q / u, swapped every iteration), two w buffers in the CT
 // layout (this iteration's w and the previous one = u_j) and z in CT.
 template <typename T>
-int lanczos_gather_impl(hubbard_model *m, const T *v0, int iters, double *alpha, double *beta, int *done,
-                        cudaStream_t st)
+int lanczos_gather_steps(hubbard_model *m, const T *v0, const LanczosPlan &P, cudaStream_t st)
 {
-    int rc = ensure_lanczos_state(m, iters, 5);
-    if (rc) return rc;
+    int rc;
     const int64_t n_p = gather_vec_elems(m);
-    const int vec_grid = (int)std::max<int64_t>(1, std::min<int64_t>((int64_t)m->sm_count * 4, (n_p + 2047) / 2048));
+    const int vec_grid = lanczos_vec_grid(m, n_p);
     if ((rc = ensure_partials(m, std::max<int64_t>(vec_grid, (int64_t)m->sm_count * 4)))) return rc;
-    T *Art = static_cast<T *>(m->work[0]), *Brt = static_cast<T *>(m->work[1]);
+    T *rt[2] = {static_cast<T *>(m->work[0]), static_cast<T *>(m->work[1])};
     T *wct[2] = {static_cast<T *>(m->work[2]), static_cast<T *>(m->work[3])};
     T *zct = static_cast<T *>(m->work[4]);
-    const double tau = m->tau >= 0 ? m->tau : (m->dtype == HUBBARD_F64 ? 1e-10 : 1e-5);
-    {
+    if (P.init) {
         ProfScope ps(m, 5, st);
-        if ((rc = launch_to_rt<T>(m, v0, Art, st))) return rc;                                      // "q_0" = f_1 unnormalised
-        CU_TRY(m, cudaMemsetAsync(Brt, 0, (size_t)n_p * sizeof(T), st));                            // line 2: f_0 <- 0
+        if ((rc = launch_to_rt<T>(m, v0, rt[0], st))) return rc;                                    // "q_0" = f_1 unnormalised
+        CU_TRY(m, cudaMemsetAsync(rt[1], 0, (size_t)n_p * sizeof(T), st));                          // line 2: f_0 <- 0
         CU_TRY(m, cudaMemsetAsync(wct[1], 0, (size_t)n_p * sizeof(T), st));
-        lanczos_scalars_init_kernel<<<1, 1, 0, st>>>(m->d_scal, tau);                               // line 1: b_1 <- 0
+        if (P.psi) CU_TRY(m, cudaMemsetAsync(P.psi, 0, (size_t)n_p * sizeof(T), st));
+        lanczos_scalars_init_kernel<<<1, 1, 0, st>>>(m->d_scal, lanczos_tau(m));                    // line 1: b_1 <- 0
         if ((rc = after_launch(m))) return rc;
     }
     GatherArgs<T> G{};
     G.S = m->d_scal; G.Zct = zct; G.alpha_out = m->d_alpha; G.beta_out = m->d_beta;
-    for (int j = 0; j < iters; ++j) {
-        G.Qrt = Art; G.Frt = Brt; G.Wct = wct[j & 1]; G.Fct = wct[(j + 1) & 1];
+    for (int j = P.j0; j < P.j1; ++j) {
+        G.Qrt = rt[j & 1]; G.Frt = rt[(j + 1) & 1]; G.Wct = wct[j & 1]; G.Fct = wct[(j + 1) & 1];
         if ((rc = launch_gather<T, false, true>(m, G, st))) return rc;     // lines 6-11 of j-1, row half of line 4
+        if (P.psi) {                                                       // f_{j+1} = c w is complete: psi += y_{j+1} f_{j+1}
+            psi_axpy_kernel<T><<<vec_grid, kVecThreads, 0, st>>>(static_cast<T *>(P.psi), G.Qrt, n_p, P.ycoef + j, m->d_scal);
+            if ((rc = after_launch(m))) return rc;
+        }
         if ((rc = launch_gather<T, true, true>(m, G, st))) return rc;      // line 4 (+ eq. 13), line 5
-        std::swap(Art, Brt);
     }
-    {
+    if (P.finish) {
         ProfScope ps(m, 3, st);
-        lanczos_final_norm_kernel<T><<<vec_grid, 512, 0, st>>>(Art, Brt, n_p, m->d_scal, m->d_partial, m->d_alpha, m->d_beta);
+        lanczos_final_norm_kernel<T><<<vec_grid, 512, 0, st>>>(rt[P.j1 & 1], rt[(P.j1 + 1) & 1], n_p, m->d_scal, m->d_partial,
+                                                               m->d_alpha, m->d_beta);
         if ((rc = after_launch(m))) return rc;
     }
-    return fetch_coefficients(m, iters, alpha, beta, done, st);
+    return HUBBARD_OK;
 }
 
+// Variants PAPER / TWOSWEEP: fused H f_j - b_j f_{j-1} with a_j, then the
+// axpy + norm sweep (kernels_lanczos.cuh); two row-major work vectors.
 template <typename T>
-int lanczos_impl(hubbard_model *m, const T *v0, int iters, double *alpha, double *beta, int *done, cudaStream_t st)
+int lanczos_classic_steps(hubbard_model *m, const T *v0, const LanczosPlan &P, cudaStream_t st)
 {
+    int rc;
     const int64_t dim = model_dim(m);
-    if (resolve_variant(m) == HUBBARD_VARIANT_GATHER) return lanczos_gather_impl<T>(m, v0, iters, alpha, beta, done, st);
-    int rc = ensure_lanczos_state(m, iters, 2);
-    if (rc) return rc;
-    const int vec_grid = (int)std::max<int64_t>(1, std::min<int64_t>((int64_t)m->sm_count * 4, (dim + 2047) / 2048));
+    const int vec_grid = lanczos_vec_grid(m, dim);
     if ((rc = ensure_partials(m, vec_grid))) return rc;
-    T *cur = static_cast<T *>(m->work[0]), *prev = static_cast<T *>(m->work[1]);
-    const double tau = m->tau >= 0 ? m->tau : (m->dtype == HUBBARD_F64 ? 1e-10 : 1e-5);
-    {
+    T *vec[2] = {static_cast<T *>(m->work[0]), static_cast<T *>(m->work[1])};
+    if (P.init) {
         ProfScope ps(m, 5, st);
-        CU_TRY(m, cudaMemcpyAsync(cur, v0, (size_t)dim * sizeof(T), cudaMemcpyDeviceToDevice, st));
-        CU_TRY(m, cudaMemsetAsync(prev, 0, (size_t)dim * sizeof(T), st));   // line 2: f_0 <- 0
+        CU_TRY(m, cudaMemcpyAsync(vec[0], v0, (size_t)dim * sizeof(T), cudaMemcpyDeviceToDevice, st));
+        CU_TRY(m, cudaMemsetAsync(vec[1], 0, (size_t)dim * sizeof(T), st));   // line 2: f_0 <- 0
+        if (P.psi) CU_TRY(m, cudaMemsetAsync(P.psi, 0, (size_t)dim * sizeof(T), st));
         CU_TRY(m, cudaMemsetAsync(m->d_scal, 0, sizeof(LanczosScalars), st));
-        lanczos_init_kernel<T><<<vec_grid, kVecThreads, 0, st>>>(cur, dim, m->d_scal, m->d_partial, tau);
+        lanczos_init_kernel<T><<<vec_grid, kVecThreads, 0, st>>>(vec[0], dim, m->d_scal, m->d_partial, lanczos_tau(m));
         if ((rc = after_launch(m))) return rc;
     }
-    for (int j = 0; j < iters; ++j) {
+    for (int j = P.j0; j < P.j1; ++j) {
+        T *cur = vec[j & 1], *prev = vec[(j + 1) & 1];
+        if (P.psi) {                                                      // f_{j+1} = c_cur * cur
+            psi_axpy_kernel<T><<<vec_grid, kVecThreads, 0, st>>>(static_cast<T *>(P.psi), cur, dim, P.ycoef + j, m->d_scal);
+            if ((rc = after_launch(m))) return rc;
+        }
         if ((rc = apply_impl<T, true>(m, cur, prev, st))) return rc;     // lines 4-5 (+ eq. 13)
         if ((rc = ensure_partials(m, vec_grid))) return rc;
         {
@@ -556,9 +594,127 @@ int lanczos_impl(hubbard_model *m, const T *v0, int iters, double *alpha, double
                                                                          m->d_alpha, m->d_beta);   // lines 6-11
             if ((rc = after_launch(m))) return rc;
         }
-        std::swap(cur, prev);
     }
+    return HUBBARD_OK;
+}
+
+template <typename T>
+int lanczos_steps(hubbard_model *m, const T *v0, const LanczosPlan &P, int coef_capacity, cudaStream_t st)
+{
+    const bool gather = resolve_variant(m) == HUBBARD_VARIANT_GATHER;
+    int rc = ensure_lanczos_state(m, coef_capacity, gather ? 5 : 2);
+    if (rc) return rc;
+    return gather ? lanczos_gather_steps<T>(m, v0, P, st) : lanczos_classic_steps<T>(m, v0, P, st);
+}
+
+template <typename T>
+int lanczos_impl(hubbard_model *m, const T *v0, int iters, double *alpha, double *beta, int *done, cudaStream_t st)
+{
+    LanczosPlan P;
+    P.j1 = iters;
+    int rc = lanczos_steps<T>(m, v0, P, iters, st);
+    if (rc) return rc;
     return fetch_coefficients(m, iters, alpha, beta, done, st);
+}
+
+// Convergence-driven stopping ("the convergence of the ground state energy can be checked after
+// each iteration"): every `check_every` iterations the coefficients so far are brought to the host and
+// E_0^(m) = lambda_min(T_m) is compared with its previous value.
+template <typename T>
+int lanczos_until_impl(hubbard_model *m, const T *v0, int max_iters, int check_every, double tol, double *alpha,
+                       double *beta, int *done, double *e0, cudaStream_t st)
+{
+    const bool gather = resolve_variant(m) == HUBBARD_VARIANT_GATHER;
+    double e_prev = 0.0, e_cur = 0.0;
+    bool have_prev = false, stopped = false;
+    int j = 0;
+    while (j < max_iters && !stopped) {
+        LanczosPlan P;
+        P.j0 = j; P.j1 = std::min(max_iters, j + check_every);
+        P.init = (j == 0); P.finish = false;
+        int rc = lanczos_steps<T>(m, v0, P, max_iters, st);
+        if (rc) return rc;
+        j = P.j1;
+        // T_j needs a_1..a_j and b_2..b_j.  GATHER has recorded j-1 pairs and holds a_j in the scalars (b_{j+1}
+        // comes with the next row sweep or the closing norm); the classic loop has recorded j pairs.
+        LanczosScalars h{};
+        CU_TRY(m, cudaMemcpyAsync(&h, m->d_scal, sizeof(h), cudaMemcpyDeviceToHost, st));
+        CU_TRY(m, cudaStreamSynchronize(st));
+        int n_rec = std::max(0, std::min(h.j, j));
+        if (n_rec > 0) {
+            CU_TRY(m, cudaMemcpy(alpha, m->d_alpha, (size_t)n_rec * sizeof(double), cudaMemcpyDeviceToHost));
+            CU_TRY(m, cudaMemcpy(beta, m->d_beta, (size_t)n_rec * sizeof(double), cudaMemcpyDeviceToHost));
+        }
+        int mm = n_rec;
+        if (h.stop) {
+            stopped = true;                                  // breakdown (Algorithm 1 lines 8-10)
+        } else if (gather && n_rec == j - 1) {
+            alpha[n_rec] = h.alpha;
+            mm = j;
+        }
+        if (mm >= 1) {
+            if (lanczos_ground_energy(alpha, beta, mm, &e_cur) != HUBBARD_OK) return HUBBARD_ERR_INVALID;
+            if (have_prev && std::fabs(e_cur - e_prev) <= tol * std::fmax(1.0, std::fabs(e_cur))) stopped = true;
+            e_prev = e_cur;
+            have_prev = true;
+        }
+    }
+    {
+        LanczosPlan P;
+        P.j0 = P.j1 = j; P.init = false; P.finish = gather;   // closing norm: b_{m+1} for the last iteration
+        int rc = lanczos_steps<T>(m, v0, P, max_iters, st);
+        if (rc) return rc;
+    }
+    int n = 0;
+    int rc = fetch_coefficients(m, max_iters, alpha, beta, &n, st);
+    if (rc) return rc;
+    if (done) *done = n;
+    if (e0) {
+        *e0 = e_cur;
+        if (n >= 1) lanczos_ground_energy(alpha, beta, n, e0);
+    }
+    return HUBBARD_OK;
+}
+
+// Ground-state vector: pass 1 = the Lanczos run, host = eigenvector y of T_m, pass 2 = the same
+// run again (bit-identical: every reduction is deterministic) accumulating psi = sum_j y_j f_j, normalised.
+template <typename T>
+int lanczos_ground_state_impl(hubbard_model *m, const T *v0, int iters, T *psi_out, double *e0, int *done, cudaStream_t st)
+{
+    std::vector<double> alpha((size_t)std::max(iters, 1)), beta((size_t)std::max(iters, 1)), y((size_t)std::max(iters, 1));
+    int n = 0;
+    int rc = lanczos_impl<T>(m, v0, iters, alpha.data(), beta.data(), &n, st);
+    if (rc) return rc;
+    if (done) *done = n;
+    if (n < 1) return HUBBARD_ERR_INVALID;
+    double lam = 0.0;
+    if ((rc = lanczos_ground_vector(alpha.data(), beta.data(), n, &lam, y.data()))) return rc;
+    if (e0) *e0 = lam;
+    const bool gather = resolve_variant(m) == HUBBARD_VARIANT_GATHER;
+    const int64_t n_vec = gather ? gather_vec_elems(m) : model_dim(m);
+    if ((rc = ensure_work(m, gather ? 6 : 2, (size_t)n_vec * sizeof(T)))) return rc;
+    if (n > m->ycoef_cap) {
+        if (m->d_ycoef) cudaFree(m->d_ycoef);
+        m->d_ycoef = nullptr; m->ycoef_cap = 0;
+        CU_TRY(m, cudaMalloc((void **)&m->d_ycoef, (size_t)n * sizeof(double)));
+        m->ycoef_cap = n;
+    }
+    CU_TRY(m, cudaMemcpyAsync(m->d_ycoef, y.data(), (size_t)n * sizeof(double), cudaMemcpyHostToDevice, st));
+    LanczosPlan P;
+    P.j1 = n; P.finish = false; P.ycoef = m->d_ycoef;
+    // GATHER accumulates in its RT layout (work[5]) and converts at the end; the classic loop is row-major already
+    P.psi = gather ? m->work[5] : static_cast<void *>(psi_out);
+    if ((rc = lanczos_steps<T>(m, v0, P, iters, st))) return rc;
+    if (gather && (rc = launch_from_rt<T>(m, static_cast<const T *>(m->work[5]), psi_out, st))) return rc;
+    const int64_t dim = model_dim(m);
+    const int vec_grid = lanczos_vec_grid(m, dim);
+    if ((rc = ensure_partials(m, vec_grid))) return rc;
+    vec_norm2_kernel<T><<<vec_grid, kVecThreads, 0, st>>>(psi_out, dim, m->d_scal, m->d_partial);
+    if ((rc = after_launch(m))) return rc;
+    vec_normalise_kernel<T><<<vec_grid, kVecThreads, 0, st>>>(psi_out, dim, m->d_scal);
+    if ((rc = after_launch(m))) return rc;
+    CU_TRY(m, cudaStreamSynchronize(st));
+    return HUBBARD_OK;
 }
 
 int ensure_stage(hubbard_model *m, int which)
@@ -610,7 +766,8 @@ void hubbard_destroy(hubbard_model *m)
     if (!m) return;
     for (auto &r : m->prof) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
     for (void *p : m->dev_allocs) cudaFree(p);
-    for (int i = 0; i < 5; ++i) if (m->work[i]) cudaFree(m->work[i]);
+    for (int i = 0; i < 6; ++i) if (m->work[i]) cudaFree(m->work[i]);
+    if (m->d_ycoef) cudaFree(m->d_ycoef);
     for (int i = 0; i < 2; ++i) if (m->stage[i]) cudaFree(m->stage[i]);
     if (m->d_scal) cudaFree(m->d_scal);
     if (m->d_partial) cudaFree(m->d_partial);
@@ -675,6 +832,38 @@ int lanczos_run(hubbard_model *m, const void *v0_dev, int iters, double *alpha_h
     if (m->dtype == HUBBARD_F32)
         return lanczos_impl<float>(m, static_cast<const float *>(v0_dev), iters, alpha_host, beta_host, iters_done, st);
     return lanczos_impl<double>(m, static_cast<const double *>(v0_dev), iters, alpha_host, beta_host, iters_done, st);
+}
+
+int lanczos_run_until(hubbard_model *m, const void *v0_dev, int max_iters, int check_every, double tol,
+                      double *alpha_host, double *beta_host, int *iters_done, double *e0, void *stream)
+{
+    int rc = check_device_model(m);
+    if (rc) return rc;
+    if (iters_done) *iters_done = 0;
+    if (!v0_dev || max_iters < 1 || check_every < 1 || !(tol >= 0.0) || !alpha_host || !beta_host) return HUBBARD_ERR_INVALID;
+    if ((uintptr_t)v0_dev & 15) return HUBBARD_ERR_INVALID;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (m->dtype == HUBBARD_F32)
+        return lanczos_until_impl<float>(m, static_cast<const float *>(v0_dev), max_iters, check_every, tol, alpha_host,
+                                         beta_host, iters_done, e0, st);
+    return lanczos_until_impl<double>(m, static_cast<const double *>(v0_dev), max_iters, check_every, tol, alpha_host,
+                                      beta_host, iters_done, e0, st);
+}
+
+int lanczos_ground_state(hubbard_model *m, const void *v0_dev, int iters, void *psi_dev, double *e0, int *iters_done,
+                         void *stream)
+{
+    int rc = check_device_model(m);
+    if (rc) return rc;
+    if (iters_done) *iters_done = 0;
+    if (!v0_dev || !psi_dev || iters < 1 || v0_dev == psi_dev) return HUBBARD_ERR_INVALID;
+    if (((uintptr_t)v0_dev | (uintptr_t)psi_dev) & 15) return HUBBARD_ERR_INVALID;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (m->dtype == HUBBARD_F32)
+        return lanczos_ground_state_impl<float>(m, static_cast<const float *>(v0_dev), iters, static_cast<float *>(psi_dev), e0,
+                                                iters_done, st);
+    return lanczos_ground_state_impl<double>(m, static_cast<const double *>(v0_dev), iters, static_cast<double *>(psi_dev), e0,
+                                             iters_done, st);
 }
 
 int hubbard_apply_host(hubbard_model *m, const void *x_host, void *y_host, void *stream)

@@ -486,6 +486,24 @@ lanczos_final_norm_kernel(const T *__restrict__ Q, const T *__restrict__ F, int6
     }
 }
 
+// The RT layout back into the caller's row-major layout (ground-state vector).
+template <typename T, int R>
+__global__ void __launch_bounds__(256)
+from_rt_kernel(const T *__restrict__ rt, T *__restrict__ x, int64_t du, int64_t dd, int64_t du_p, int64_t dd_p)
+{
+    using PR = Pack<T, R>;
+    const int64_t n = du_p / R * dd_p;
+    for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p < n; p += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t tile = p / dd_p, b = p - tile * dd_p;
+        const PR v = reinterpret_cast<const PR *>(rt)[p];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int64_t a = tile * R + r;
+            if (a < du && b < dd) x[a * dd + b] = v.v[r];
+        }
+    }
+}
+
 __global__ void lanczos_scalars_init_kernel(LanczosScalars *S, double tau)
 {
     S->c_cur = 0.0; S->c_prev = 0.0; S->beta = 0.0; S->alpha = 0.0; S->amax = 0.0; S->tau = tau;

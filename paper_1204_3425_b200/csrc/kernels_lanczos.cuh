@@ -114,4 +114,44 @@ lanczos_axpy_norm_kernel(const T *__restrict__ u, T *__restrict__ w, int64_t dim
     }
 }
 
+// ---- ground-state vector (second Lanczos pass, "the basis is not kept")
+// psi += y_j f_j with f_j = c_cur * u (the scalars are those of the run in flight).
+template <typename T>
+__global__ void __launch_bounds__(kVecThreads)
+psi_axpy_kernel(T *__restrict__ psi, const T *__restrict__ u, int64_t n, const double *__restrict__ ycoef,
+                const LanczosScalars *S)
+{
+    if (S->stop) return;
+    const T a = (T)(*ycoef * S->c_cur);
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
+        psi[i] = fma(a, u[i], psi[i]);
+}
+
+// |x|^2 into S->beta (deterministic, as every other reduction here), then x *= 1 / sqrt(S->beta).
+template <typename T>
+__global__ void __launch_bounds__(kVecThreads)
+vec_norm2_kernel(const T *__restrict__ x, int64_t n, LanczosScalars *S, double *partials)
+{
+    __shared__ double red[32];
+    __shared__ int flag;
+    double acc = 0.0;
+    const int64_t per = (n + gridDim.x - 1) / gridDim.x;
+    const int64_t lo = blockIdx.x * per, hi = min(n, lo + per);
+    for (int64_t i = lo + threadIdx.x; i < hi; i += blockDim.x) acc += (double)x[i] * (double)x[i];
+    const double s = block_sum(acc, red);
+    if (publish_and_check_last(s, partials, blockIdx.x, gridDim.x, &S->ticket, &flag)) {
+        const double tot = sum_partials(partials, gridDim.x, red);
+        if (threadIdx.x == 0) { S->beta = tot; S->ticket = 0; }
+    }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(kVecThreads)
+vec_normalise_kernel(T *__restrict__ x, int64_t n, const LanczosScalars *S)
+{
+    const double n2 = S->beta;
+    const T a = (T)((n2 > 0.0) ? rsqrt(n2) : 0.0);
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) x[i] *= a;
+}
+
 }  // namespace hub

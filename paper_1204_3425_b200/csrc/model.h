@@ -86,8 +86,10 @@ struct hubbard_model {
     hub::DevModel dev{};
     std::vector<void *> dev_allocs;    // everything to cudaFree
     // Lanczos state (allocated on first use)
-    void *work[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // 2 (PAPER/TWOSWEEP) or 5 (GATHER) in use
-    size_t work_bytes[5] = {0, 0, 0, 0, 0};
+    void *work[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // 2 (PAPER/TWOSWEEP) or 5 (GATHER) in use, [5]: psi
+    size_t work_bytes[6] = {0, 0, 0, 0, 0, 0};
+    double *d_ycoef = nullptr;         // eigenvector of T_m for the ground-state pass
+    int ycoef_cap = 0;
     hub::LanczosScalars *d_scal = nullptr;
     double *d_partial = nullptr;       // per-block partial sums
     int64_t n_partial = 0;

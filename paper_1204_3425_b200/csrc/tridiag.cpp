@@ -3,6 +3,7 @@
 #include <cmath>
 #include <cstdint>
 #include <limits>
+#include <new>
 
 #include "../../include/hubbard.h"
 
@@ -47,5 +48,73 @@ extern "C" int lanczos_ground_energy(const double *alpha, const double *beta, in
         if (sturm_count(alpha, beta, m, mid) >= 1) hi = mid; else lo = mid;
     }
     *e0 = 0.5 * (lo + hi);
+    return HUBBARD_OK;
+}
+
+// Eigenvector of T_m for its smallest eigenvalue ("the
+// eigenvalues and eigenvectors of T can be computed with standard methods"):
+// inverse iteration on (T - sigma I) with sigma just below the bisection value,
+// tridiagonal LU with partial pivoting, three sweeps.  y has unit norm and
+// y[0] >= 0.
+extern "C" int lanczos_ground_vector(const double *alpha, const double *beta, int m, double *e0, double *y)
+{
+    if (!y) return HUBBARD_ERR_INVALID;
+    double lam = 0.0;
+    int rc = lanczos_ground_energy(alpha, beta, m, &lam);
+    if (rc) return rc;
+    if (e0) *e0 = lam;
+    if (m == 1) { y[0] = 1.0; return HUBBARD_OK; }
+    double scale = 0.0;
+    for (int i = 0; i < m; ++i) scale = std::fmax(scale, std::fabs(alpha[i]) + (i + 1 < m ? std::fabs(beta[i]) : 0.0));
+    const double sigma = lam - 1e-13 * std::fmax(scale, 1.0);
+    double *buf = new (std::nothrow) double[5 * (size_t)m];
+    if (!buf) return HUBBARD_ERR_HOST_OOM;
+    double *d = buf, *u1 = buf + m, *u2 = buf + 2 * m, *l = buf + 3 * m, *rhs = buf + 4 * m;
+    int *piv = new (std::nothrow) int[(size_t)m];
+    if (!piv) { delete[] buf; return HUBBARD_ERR_HOST_OOM; }
+    // LU of the shifted matrix: rows are (sub, diag, super); after elimination row i holds d[i], u1[i], u2[i]
+    for (int i = 0; i < m; ++i) { d[i] = alpha[i] - sigma; u1[i] = (i + 1 < m) ? beta[i] : 0.0; u2[i] = 0.0; }
+    const double tiny = 1e-300 + 1e-16 * std::fmax(scale, 1.0);
+    for (int i = 0; i + 1 < m; ++i) {
+        const double sub = beta[i];                 // element (i+1, i)
+        if (std::fabs(sub) > std::fabs(d[i])) {     // swap rows i and i+1
+            piv[i] = 1;
+            const double di = d[i], ui = u1[i];
+            d[i] = sub; u1[i] = d[i + 1]; u2[i] = u1[i + 1];
+            l[i] = di / sub;
+            d[i + 1] = ui - l[i] * u1[i];
+            u1[i + 1] = -l[i] * u2[i];
+        } else {
+            piv[i] = 0;
+            if (d[i] == 0.0) d[i] = tiny;
+            l[i] = sub / d[i];
+            d[i + 1] -= l[i] * u1[i];
+        }
+    }
+    if (d[m - 1] == 0.0) d[m - 1] = tiny;
+    for (int i = 0; i < m; ++i) y[i] = 1.0 / std::sqrt((double)m) * (1.0 + 0.01 * ((i * 7) % 5));
+    for (int sweep = 0; sweep < 3; ++sweep) {
+        for (int i = 0; i < m; ++i) rhs[i] = y[i];
+        for (int i = 0; i + 1 < m; ++i) {           // forward: apply the row operations
+            if (piv[i]) { const double t = rhs[i]; rhs[i] = rhs[i + 1]; rhs[i + 1] = t; }
+            rhs[i + 1] -= l[i] * rhs[i];
+        }
+        for (int i = m - 1; i >= 0; --i) {          // back substitution
+            double s = rhs[i];
+            if (i + 1 < m) s -= u1[i] * y[i + 1];
+            if (i + 2 < m) s -= u2[i] * y[i + 2];
+            y[i] = s / d[i];
+        }
+        double nrm = 0.0;
+        for (int i = 0; i < m; ++i) nrm = std::fmax(nrm, std::fabs(y[i]));
+        if (!(nrm > 0.0) || !std::isfinite(nrm)) { delete[] buf; delete[] piv; return HUBBARD_ERR_INVALID; }
+        for (int i = 0; i < m; ++i) y[i] /= nrm;
+    }
+    double n2 = 0.0;
+    for (int i = 0; i < m; ++i) n2 += y[i] * y[i];
+    const double s = (y[0] < 0.0 ? -1.0 : 1.0) / std::sqrt(n2);
+    for (int i = 0; i < m; ++i) y[i] *= s;
+    delete[] buf;
+    delete[] piv;
     return HUBBARD_OK;
 }

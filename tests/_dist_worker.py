@@ -17,7 +17,8 @@ t = bench.max_over_ranks(10.0 + rank, world, torch.device("cpu"))
 # replicas: per-rank work is fixed, the aggregate is world x the per-rank rate at the max time
 iters_per_rank = 200
 value = world * iters_per_rank / t
-print(json.dumps({"rank": rank, "world": world, "local": local, "t_max": t, "value": value}), flush=True)
+sys.stdout.write(json.dumps({"rank": rank, "world": world, "local": local, "t_max": t, "value": value}) + "\n")
+sys.stdout.flush()
 if world > 1:
     import torch.distributed as dist
     dist.destroy_process_group()

@@ -194,3 +194,21 @@ def test_gather_table_is_a_bank_aware_permutation_of_the_hops(name, ns, nu, nd, 
                     worst += len(banks) - len(np.unique(banks))
             assert worst <= conflicts
             assert conflicts <= max(4, n_real // 200)
+
+
+def test_ground_vector_vs_lapack():
+    """Host utility: lowest eigenpair of T_m against LAPACK's dense solver, including a
+    nearly-degenerate pair and tiny off-diagonals."""
+    rng = np.random.default_rng(7)
+    cases = [(rng.normal(size=m), np.abs(rng.normal(size=m - 1)) + 0.1) for m in (2, 3, 17, 200)]
+    cases.append((np.array([1.0, 1.0 + 1e-9, 3.0]), np.array([1e-7, 0.5])))
+    cases.append((np.array([2.0]), np.zeros(0)))
+    for a, b in cases:
+        e0, y = hb.lanczos_ground_vector(a, b)
+        T = np.diag(a) + np.diag(b, 1) + np.diag(b, -1) if len(a) > 1 else np.array([[a[0]]])
+        w, v = np.linalg.eigh(T)
+        assert abs(e0 - w[0]) <= 1e-12 * max(1.0, np.max(np.abs(w)))
+        assert abs(np.linalg.norm(y) - 1.0) < 1e-12 and y[0] >= 0.0
+        assert np.max(np.abs(T @ y - e0 * y)) <= 1e-10 * max(1.0, np.max(np.abs(w)))
+        if len(a) > 1 and w[1] - w[0] > 1e-6:
+            assert abs(abs(np.dot(y, v[:, 0])) - 1.0) < 1e-8

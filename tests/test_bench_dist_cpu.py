@@ -24,12 +24,18 @@ def _torchrun(script_args, nproc=2, timeout=300):
 
 
 def _json_lines(text):
-    out = []
-    for line in text.splitlines():
-        line = line.strip()
-        if line.startswith("{"):
-            out.append(json.loads(line))
-    return out
+    """Every top-level JSON object in `text` (two ranks may interleave their lines on one stdout)."""
+    out, dec, i = [], json.JSONDecoder(), 0
+    while True:
+        i = text.find("{", i)
+        if i < 0:
+            return out
+        try:
+            obj, end = dec.raw_decode(text, i)
+            out.append(obj)
+            i = end
+        except json.JSONDecodeError:
+            i += 1
 
 
 def test_replica_timing_logic_world2_gloo():

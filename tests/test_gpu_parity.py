@@ -341,3 +341,84 @@ def test_non_default_stream():
     s.synchronize()
     torch.cuda.synchronize()
     assert torch.equal(y0, y1)
+
+
+# ---------------------------------------------------------------- SURVEY 8(f)-2
+def _double_occupancy(psi_np, st_up, st_dn):
+    docc = np.array([[bin(int(u) & int(d)).count("1") for d in st_dn] for u in st_up], dtype=np.float64)
+    return float(np.sum(docc.reshape(-1) * psi_np * psi_np))
+
+
+@pytest.mark.parametrize("variant", ["paper", "twosweep", "gather"])
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_ground_state_vector_small(dtype, variant):
+    """lanczos_ground_state against the dense eigenvector of the definitional H (tier 0) on a sector with a
+    non-degenerate ground state: overlap, energy, residual |H psi - E psi| and the double occupancy
+    <sum_i n_iup n_idn> (eq. 2)."""
+    ns, nu, nd, bonds, t, U = 6, 3, 3, ring_bonds(6), 1.0, 4.0
+    H = hd.dense_hamiltonian(ns, nu, nd, bonds, t, U)
+    w, v = np.linalg.eigh(H)
+    assert w[1] - w[0] > 1e-3
+    m = hb.hubbard_create(ns, nu, nd, bonds, t, U, dtype)
+    m.hubbard_set_variant(VARIANTS[variant])
+    v0, _ = start_vector(11, m.dim, dtype)
+    psi = torch.empty_like(v0)
+    e0, done = m.lanczos_ground_state(v0, 80, psi)
+    tol = 1e-9 if dtype == "f64" else 2e-4
+    assert abs(e0 - w[0]) <= (1e-10 if dtype == "f64" else 1e-5) * abs(w[0])
+    p = psi.double().cpu().numpy()
+    assert abs(np.linalg.norm(p) - 1.0) < (1e-12 if dtype == "f64" else 1e-6)
+    assert abs(abs(np.dot(p, v[:, 0])) - 1.0) <= tol
+    assert np.max(np.abs(H @ p - e0 * p)) <= (1e-7 if dtype == "f64" else 1e-3)
+    st_up, st_dn = m.hubbard_get_basis(0), m.hubbard_get_basis(1)
+    # an observable is linear in the vector error (the overlap is quadratic in it)
+    assert abs(_double_occupancy(p, st_up, st_dn) - _double_occupancy(v[:, 0], st_up, st_dn)) <= (1e-6 if dtype == "f64" else 2e-3)
+
+
+def test_ground_state_vector_C2_vs_oracle_eigsh():
+    """C2 (dim 853 776): the ground vector from the CUDA path against the oracle's matrix-free H with a
+    library eigensolver (scipy ARPACK on oracle.ref.RefModel.apply)."""
+    from scipy.sparse.linalg import LinearOperator, eigsh
+    c = CONFIGS["C2"]
+    ref = RefModel(c.n_sites, c.n_up, c.n_dn, c.bonds, c.t, 4.0)
+    m = hb.hubbard_create(c.n_sites, c.n_up, c.n_dn, c.bonds, c.t, 4.0, "f64")
+    v0, v0_np = start_vector(c.seed, c.dim, "f64")
+    psi = torch.empty_like(v0)
+    e0, done = m.lanczos_ground_state(v0, 200, psi)
+    assert done == 200
+    w, v = eigsh(LinearOperator((c.dim, c.dim), matvec=ref.apply, dtype=np.float64), k=1, which="SA", v0=v0_np, tol=1e-12)
+    assert abs(e0 - w[0]) <= 1e-10 * abs(w[0])
+    p = psi.double().cpu().numpy()
+    assert abs(abs(np.dot(p, v[:, 0])) - 1.0) <= 1e-8
+    # the library's own H on its own vector: Rayleigh quotient = E_0, small residual
+    hp = torch.empty_like(psi)
+    m.hubbard_apply(psi, hp)
+    torch.cuda.synchronize()
+    assert abs(torch.dot(psi, hp).item() - e0) <= 1e-10 * abs(e0)
+    assert (hp - e0 * psi).abs().max().item() <= 1e-6
+
+
+@pytest.mark.parametrize("variant", ["twosweep", "gather"])
+def test_run_until_converges_and_matches_fixed_run(variant):
+    """Convergence-driven stopping: stops well before the iteration cap, returns the same
+    alpha/beta as a fixed run of that length (bit-identical: same kernels, same order) and E_0 within tol."""
+    c = CONFIGS["C2"]
+    m = hb.hubbard_create(c.n_sites, c.n_up, c.n_dn, c.bonds, c.t, 4.0, "f64")
+    m.hubbard_set_variant(VARIANTS[variant])
+    v0, _ = start_vector(c.seed, c.dim, "f64")
+    a, b, e0 = m.lanczos_run_until(v0, 400, check_every=10, tol=1e-11)
+    n = len(a)
+    assert 30 <= n < 400 and n % 10 == 0
+    a2, b2 = m.lanczos_run(v0, n)
+    assert np.array_equal(a, a2) and np.array_equal(b, b2)
+    assert abs(e0 - hb.lanczos_ground_energy(a, b)) == 0.0
+    assert abs(e0 - (-6.920353562419)) < 1e-8                        # SURVEY P11 / oracle test_P11_C2_energy
+    # the cap is honoured and a breakdown ends the run (t = 0)
+    a3, b3, _ = m.lanczos_run_until(v0, 25, check_every=10, tol=0.0)
+    assert len(a3) == 25
+    m0 = hb.hubbard_create(6, 3, 3, ring_bonds(6), 0.0, 4.0, "f64")
+    m0.hubbard_set_variant(VARIANTS[variant])
+    x, _ = start_vector(5, m0.dim, "f64")
+    a4, b4, e4 = m0.lanczos_run_until(x, 50, check_every=3, tol=0.0)
+    a5, b5 = m0.lanczos_run(x, 50)
+    assert len(a4) == len(a5) < 50 and abs(e4) < 1e-9
