@@ -62,11 +62,14 @@ enum {
     HUBBARD_VARIANT_PAPER = 1,   /* Algorithms 2-4 restated: one thread per element, one fused kernel */
     HUBBARD_VARIANT_TWOSWEEP = 2,/* row sweep (down term + diagonal, row staged in shared memory)
                                     + strip sweep (up term over L2-resident column strips) */
-    HUBBARD_VARIANT_GATHER = 3   /* symmetric gather sweeps: R whole rows (down term) then R whole
+    HUBBARD_VARIANT_GATHER = 3,  /* symmetric gather sweeps: R whole rows (down term) then R whole
                                     columns (up term) staged interleaved in shared memory; in
                                     lanczos_run the vector updates are folded into the two sweeps
                                     (five work vectors in tile-major layouts).  INVALID if a row or column of V
                                     does not fit in shared memory. */
+    HUBBARD_VARIANT_PERSIST = 4  /* small sectors: the whole Lanczos loop in ONE cooperative kernel, the two
+                                    reductions of an iteration as grid-wide barriers (plain hubbard_apply uses
+                                    the PAPER kernel).  AUTO picks it for dim <= 2^17. */
 };
 
 /* ---- construction ("first, we prepare the data on the host") ----

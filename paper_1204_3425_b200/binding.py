@@ -13,7 +13,7 @@ import numpy as np
 from . import build as _build
 
 HUBBARD_F32, HUBBARD_F64 = 0, 1
-VARIANT_AUTO, VARIANT_PAPER, VARIANT_TWOSWEEP, VARIANT_GATHER = 0, 1, 2, 3
+VARIANT_AUTO, VARIANT_PAPER, VARIANT_TWOSWEEP, VARIANT_GATHER, VARIANT_PERSIST = 0, 1, 2, 3, 4
 N_KCLASS = 6
 KCLASS_NAMES = ("hv_paper", "row_sweep", "col_sweep", "vec_sweep", "scalar", "setup")
 

@@ -81,6 +81,7 @@ struct hubbard_model {
     int64_t launches = 0;
     int sm_count = 148;
     int max_smem_optin = 0;
+    int coop_launch = 0;               // device supports cooperative launches (variant PERSIST)
     int gather_R = 0;                  // tile height of variant GATHER, 0 = does not fit
 
     hub::DevModel dev{};
