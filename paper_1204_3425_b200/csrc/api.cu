@@ -463,8 +463,17 @@ int apply_impl(hubbard_model *m, const T *x, T *y, cudaStream_t st)
         return launch_gather<T, true, false>(m, G, st);
     }
     SweepArgs<T> A{x, y, LZ ? m->d_scal : nullptr, m->d_partial};
-    int rc = m->dev.dn_ent16 ? launch_row<T, uint16_t, LZ>(m, A, m->dev.dn_ent16, st)
+    int rc;
+    if (m->variant == HUBBARD_VARIANT_AUTO && gather_R(m) > 0 && !env_int("HUBBARD_TWOSWEEP_OLD_ROW", 0)) {
+        // AUTO fell back to TWOSWEEP because the tile is narrower than 16 bytes (C5 fp32): the row half still runs
+        // as the gather ROW sweep on row-major vectors (batch-interleaved, bank-aware tables; vectorised staging)
+        GatherArgs<T> G{};
+        G.x = x; G.y = y; G.y_rowmajor = 1; G.S = LZ ? m->d_scal : nullptr;
+        rc = launch_gather<T, false, false>(m, G, st);
+    } else {
+        rc = m->dev.dn_ent16 ? launch_row<T, uint16_t, LZ>(m, A, m->dev.dn_ent16, st)
                              : launch_row<T, uint32_t, LZ>(m, A, m->dev.dn_ent32, st);
+    }
     if (rc) return rc;
     return launch_strip<T, LZ>(m, A, st);
 }

@@ -234,6 +234,12 @@ gather_sweep_kernel(GatherArgs<T> A)
             bcp = (T)(A.S->beta * A.S->c_prev);           // b_{j+1} f_j = (b_{j+1} c_j) u_j
         }
     }
+    if (!LZ && !COL && A.y_rowmajor && A.S) {
+        // classic (three-kernel) Lanczos form on row-major vectors: y = c (t H_dn + D) x - b_j c_{j-1} y  (eq. 13, row half)
+        if (A.S->stop) return;
+        c = (T)A.S->c_cur;
+        bcp = (T)(A.S->beta * A.S->c_prev);
+    }
     if (threadIdx.x < kZeroSlots) {
         PR z;
 #pragma unroll
@@ -396,7 +402,10 @@ gather_sweep_kernel(GatherArgs<T> A)
                     if (valid) {
 #pragma unroll
                         for (int r = 0; r < R; ++r)
-                            if (o0 + r < du) A.y[(o0 + r) * dd + i] = h[r];
+                            if (o0 + r < du) {
+                                const int64_t J = (o0 + r) * dd + i;
+                                A.y[J] = A.S ? c * h[r] - bcp * A.y[J] : h[r];
+                            }
                     }
                 } else {
                     const PR wt = block_transpose<T, R>(xi.v, q);
