@@ -430,3 +430,20 @@ def test_run_until_converges_and_matches_fixed_run(variant):
     a4, b4, e4 = m0.lanczos_run_until(x, 50, check_every=3, tol=0.0)
     a5, b5 = m0.lanczos_run(x, 50)
     assert len(a4) == len(a5) < 50 and abs(e4) < 1e-9
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_lanczos_C4_prefix_vs_oracle(dtype):
+    """Headline configuration at full size in the launch configuration bench.py times (variant AUTO = the two
+    gather sweeps): the first Lanczos coefficients against Algorithm 1 run verbatim on the tier-1 oracle's H*v."""
+    c = CONFIGS["C4"]
+    n = 6
+    ref = RefModel(c.n_sites, c.n_up, c.n_dn, c.bonds, c.t, 8.0)
+    m = hb.hubbard_create(c.n_sites, c.n_up, c.n_dn, c.bonds, c.t, 8.0, dtype)
+    v0, v0_np = start_vector(c.seed, c.dim, dtype)
+    alpha, beta = m.lanczos_run(v0, n)
+    a_ref, b_ref = lr.lanczos(ref.apply, v0_np, n)
+    tol = 1e-10 if dtype == "f64" else 1e-5
+    assert len(alpha) == n
+    assert np.max(np.abs(alpha - a_ref) / np.maximum(1.0, np.abs(a_ref))) <= tol
+    assert np.max(np.abs(beta - b_ref) / np.maximum(1.0, np.abs(b_ref))) <= tol
