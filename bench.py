@@ -32,9 +32,9 @@ UNIT = "Hv/s"
 FALLBACK_HBM_GBS = 6650.0      # /opt/skills/guides/B200_PROFILING.md fallback
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures
 # (profiles/*_ncu_full.md name the command); keyed by (config, dtype, kernel class).
-NCU_TRAFFIC = {   # profiles/r01e_gather_c4_ncu_full.md
-    ("C4", "f64", "row_sweep"): 7.6427e9, ("C4", "f64", "col_sweep"): 5.7103e9,
-    ("C4", "f32", "row_sweep"): 3.7615e9, ("C4", "f32", "col_sweep"): 2.8305e9,
+NCU_TRAFFIC = {   # profiles/r01g_final_gather_c4_ncu_full.md
+    ("C4", "f64", "row_sweep"): 6.7461e9, ("C4", "f64", "col_sweep"): 5.5661e9,
+    ("C4", "f32", "row_sweep"): 3.3439e9, ("C4", "f32", "col_sweep"): 2.5984e9,
 }
 
 
