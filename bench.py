@@ -333,8 +333,13 @@ def run_native_dtype(args, cfg, U, dtype, rank, world, local):
         m.hubbard_apply(psi, hp, stream)
         torch.cuda.synchronize()
         resid = float((hp - e_gs * psi).abs().max().item())
+        t0 = time.perf_counter()
+        n_pr = m.lanczos_propagate(v0, 30, 0.0, 0.05, psi, hp, stream)      # exp(-i 0.05 H) v0, 30 Krylov vectors
+        t_pr = time.perf_counter() - t0
+        nrm = float(torch.sqrt((psi.double() ** 2).sum() + (hp.double() ** 2).sum()).item())
         nxt = {"run_until": {"tol": 1e-12, "check_every": 10, "iters_done": len(a_u), "E0": e_u, "s": t_until},
-               "ground_state": {"iters": n_gs, "E0": e_gs, "s": t_gs, "max_abs_residual": resid}}
+               "ground_state": {"iters": n_gs, "E0": e_gs, "s": t_gs, "max_abs_residual": resid},
+               "propagate": {"iters": n_pr, "t": 0.05, "s": t_pr, "norm_after": nrm}}
         del psi, hp
 
     # ---- end to end: host start vector (pinned) -> lanczos_run_host -> alpha/beta on the host

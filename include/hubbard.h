@@ -166,6 +166,15 @@ int lanczos_run_until(hubbard_model *m, const void *v0_dev, int max_iters, int c
 int lanczos_ground_state(hubbard_model *m, const void *v0_dev, int iters, void *psi_dev, double *e0, int *iters_done,
                          void *stream);
 
+/* lanczos_propagate: Krylov (Lanczos) propagation with the same H v ("time propagation"):
+ *   out = exp(-(tau + i t) H) v0  ~  |v0| V_m exp(-(tau + i t) T_m) e_1,   m = iters (fewer on breakdown)
+ * for a REAL start vector v0 (tau: imaginary time, t: real time).  out_re_dev / out_im_dev: device, dim elements
+ * of the model's dtype, row-major, caller-owned, distinct from v0 and from each other; out_im_dev may be NULL
+ * (e.g. t == 0).  Pass 1 is lanczos_run, the host exponentiates T_m (full tridiagonal eigen-decomposition), each
+ * output part is one more identical run accumulating sum_j y_j f_j.  Synchronises the stream. */
+int lanczos_propagate(hubbard_model *m, const void *v0_dev, int iters, double tau, double t, void *out_re_dev,
+                      void *out_im_dev, int *iters_done, void *stream);
+
 /* Breakdown threshold tau (>= 0; 0 = the paper's literal "b = 0" test). */
 int lanczos_set_tau(hubbard_model *m, double tau);
 
@@ -215,6 +224,8 @@ int hubbard_get_gather_table(const hubbard_model *m, int spin, int lanes, int64_
 int lanczos_ground_energy(const double *alpha, const double *beta, int m, double *e0);
 /* Same, plus the eigenvector y (m doubles, unit norm, y[0] >= 0) of that eigenvalue (inverse iteration); e0 may be NULL. */
 int lanczos_ground_vector(const double *alpha, const double *beta, int m, double *e0, double *y);
+/* y = exp(-(tau + i t) T_m) e_1 as real and imaginary parts (m doubles each); host, O(m^3). */
+int lanczos_expm_e1(const double *alpha, const double *beta, int m, double tau, double t, double *y_re, double *y_im);
 
 /* ---- measurement hooks ----
  * hubbard_profile(m, 1) makes every later kernel launch of this model be

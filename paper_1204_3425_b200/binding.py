@@ -20,7 +20,7 @@ KCLASS_NAMES = ("hv_paper", "row_sweep", "col_sweep", "vec_sweep", "scalar", "se
 ABI_SYMBOLS = (
     "hubbard_create", "hubbard_create_host", "hubbard_destroy", "hubbard_dims", "hubbard_set_U",
     "hubbard_set_variant", "hubbard_apply", "lanczos_run", "lanczos_run_until", "lanczos_ground_state",
-    "lanczos_ground_vector", "lanczos_set_tau", "hubbard_apply_host",
+    "lanczos_ground_vector", "lanczos_propagate", "lanczos_expm_e1", "lanczos_set_tau", "hubbard_apply_host",
     "lanczos_run_host", "hubbard_get_basis", "hubbard_get_hops", "hubbard_get_gather_table", "lanczos_ground_energy",
     "hubbard_profile", "hubbard_kernel_times", "hubbard_launch_count", "hubbard_last_cuda_error",
     "hubbard_strerror",
@@ -50,6 +50,8 @@ def _load() -> C.CDLL:
     lib.lanczos_run_until.argtypes = [vp, vp, i32, i32, dbl, P(dbl), P(dbl), P(i32), P(dbl), vp]
     lib.lanczos_ground_state.argtypes = [vp, vp, i32, vp, P(dbl), P(i32), vp]
     lib.lanczos_ground_vector.argtypes = [P(dbl), P(dbl), i32, P(dbl), P(dbl)]
+    lib.lanczos_propagate.argtypes = [vp, vp, i32, dbl, dbl, vp, vp, P(i32), vp]
+    lib.lanczos_expm_e1.argtypes = [P(dbl), P(dbl), i32, dbl, dbl, P(dbl), P(dbl)]
     lib.hubbard_apply_host.argtypes = [vp, vp, vp, vp]
     lib.lanczos_run_host.argtypes = [vp, vp, i32, P(dbl), P(dbl), P(i32), vp]
     lib.hubbard_get_basis.argtypes = [vp, i32, P(C.c_uint32)]
@@ -183,6 +185,14 @@ class Model:
                "lanczos_ground_state", self._h)
         return e0.value, done.value
 
+    def lanczos_propagate(self, v0, iters, tau, t, out_re, out_im=None, stream=None):
+        """out = exp(-(tau + i t) H) v0 by Krylov propagation (real v0); returns the iterations done."""
+        done = C.c_int(0)
+        _check(lib.lanczos_propagate(self._h, _dptr(v0), iters, float(tau), float(t), _dptr(out_re),
+                                     _dptr(out_im) if out_im is not None else None, C.byref(done), _stream(stream)),
+               "lanczos_propagate", self._h)
+        return done.value
+
     # -- hot path, host buffers (numpy arrays or CPU torch tensors)
     @staticmethod
     def _hptr(a) -> int:
@@ -290,3 +300,17 @@ def lanczos_ground_vector(alpha, beta, m=None):
     _check(lib.lanczos_ground_vector(a.ctypes.data_as(dp), b.ctypes.data_as(dp), m, C.byref(e0), y.ctypes.data_as(dp)),
            "lanczos_ground_vector")
     return e0.value, y
+
+
+def lanczos_expm_e1(alpha, beta, tau, t, m=None):
+    """exp(-(tau + i t) T_m) e_1 as a complex numpy vector (host utility)."""
+    a = np.ascontiguousarray(alpha, dtype=np.float64)
+    b = np.ascontiguousarray(beta, dtype=np.float64)
+    m = len(a) if m is None else int(m)
+    if len(b) == 0:
+        b = np.zeros(1)
+    yr, yi = np.zeros(m), np.zeros(m)
+    dp = C.POINTER(C.c_double)
+    _check(lib.lanczos_expm_e1(a.ctypes.data_as(dp), b.ctypes.data_as(dp), m, float(tau), float(t), yr.ctypes.data_as(dp),
+                               yi.ctypes.data_as(dp)), "lanczos_expm_e1")
+    return yr + 1j * yi

@@ -727,8 +727,33 @@ int lanczos_until_impl(hubbard_model *m, const T *v0, int max_iters, int check_e
     return HUBBARD_OK;
 }
 
-// Ground-state vector: pass 1 = the Lanczos run, host = eigenvector y of T_m, pass 2 = the same
-// run again (bit-identical: every reduction is deterministic) accumulating psi = sum_j y_j f_j, normalised.
+// Second Lanczos pass: out = sum_j y_j f_j (row-major, not normalised) for host coefficients y[0..n).  The run
+// is bit-identical to the one that produced T_n (every reduction is deterministic), so the f_j are the same.
+template <typename T>
+int lanczos_combine(hubbard_model *m, const T *v0, int n, const double *y_host, T *out, cudaStream_t st)
+{
+    const bool gather = resolve_variant(m) == HUBBARD_VARIANT_GATHER;
+    const int64_t n_vec = gather ? gather_vec_elems(m) : model_dim(m);
+    int rc = ensure_work(m, gather ? 6 : 2, (size_t)n_vec * sizeof(T));
+    if (rc) return rc;
+    if (n > m->ycoef_cap) {
+        if (m->d_ycoef) cudaFree(m->d_ycoef);
+        m->d_ycoef = nullptr; m->ycoef_cap = 0;
+        CU_TRY(m, cudaMalloc((void **)&m->d_ycoef, (size_t)n * sizeof(double)));
+        m->ycoef_cap = n;
+    }
+    CU_TRY(m, cudaMemcpyAsync(m->d_ycoef, y_host, (size_t)n * sizeof(double), cudaMemcpyHostToDevice, st));
+    LanczosPlan P;
+    P.j1 = n; P.finish = false; P.ycoef = m->d_ycoef;
+    // GATHER accumulates in its RT layout (work[5]) and converts at the end; the other loops are row-major already
+    P.psi = gather ? m->work[5] : static_cast<void *>(out);
+    if ((rc = lanczos_steps<T>(m, v0, P, n, st))) return rc;
+    if (gather && (rc = launch_from_rt<T>(m, static_cast<const T *>(m->work[5]), out, st))) return rc;
+    CU_TRY(m, cudaStreamSynchronize(st));      // y_host may go out of scope in the caller
+    return HUBBARD_OK;
+}
+
+// Ground-state vector: pass 1 = the Lanczos run, host = eigenvector y of T_m, pass 2 = combine.
 template <typename T>
 int lanczos_ground_state_impl(hubbard_model *m, const T *v0, int iters, T *psi_out, double *e0, int *done, cudaStream_t st)
 {
@@ -741,22 +766,7 @@ int lanczos_ground_state_impl(hubbard_model *m, const T *v0, int iters, T *psi_o
     double lam = 0.0;
     if ((rc = lanczos_ground_vector(alpha.data(), beta.data(), n, &lam, y.data()))) return rc;
     if (e0) *e0 = lam;
-    const bool gather = resolve_variant(m) == HUBBARD_VARIANT_GATHER;
-    const int64_t n_vec = gather ? gather_vec_elems(m) : model_dim(m);
-    if ((rc = ensure_work(m, gather ? 6 : 2, (size_t)n_vec * sizeof(T)))) return rc;
-    if (n > m->ycoef_cap) {
-        if (m->d_ycoef) cudaFree(m->d_ycoef);
-        m->d_ycoef = nullptr; m->ycoef_cap = 0;
-        CU_TRY(m, cudaMalloc((void **)&m->d_ycoef, (size_t)n * sizeof(double)));
-        m->ycoef_cap = n;
-    }
-    CU_TRY(m, cudaMemcpyAsync(m->d_ycoef, y.data(), (size_t)n * sizeof(double), cudaMemcpyHostToDevice, st));
-    LanczosPlan P;
-    P.j1 = n; P.finish = false; P.ycoef = m->d_ycoef;
-    // GATHER accumulates in its RT layout (work[5]) and converts at the end; the classic loop is row-major already
-    P.psi = gather ? m->work[5] : static_cast<void *>(psi_out);
-    if ((rc = lanczos_steps<T>(m, v0, P, iters, st))) return rc;
-    if (gather && (rc = launch_from_rt<T>(m, static_cast<const T *>(m->work[5]), psi_out, st))) return rc;
+    if ((rc = lanczos_combine<T>(m, v0, n, y.data(), psi_out, st))) return rc;
     const int64_t dim = model_dim(m);
     const int vec_grid = lanczos_vec_grid(m, dim);
     if ((rc = ensure_partials(m, vec_grid))) return rc;
@@ -765,6 +775,35 @@ int lanczos_ground_state_impl(hubbard_model *m, const T *v0, int iters, T *psi_o
     vec_normalise_kernel<T><<<vec_grid, kVecThreads, 0, st>>>(psi_out, dim, m->d_scal);
     if ((rc = after_launch(m))) return rc;
     CU_TRY(m, cudaStreamSynchronize(st));
+    return HUBBARD_OK;
+}
+
+// Krylov propagation: exp(-(tau + i t) H) v0 ~ |v0| V_m exp(-(tau + i t) T_m) e_1 for a
+// REAL start vector; the real and the imaginary part are each one combine pass.
+template <typename T>
+int lanczos_propagate_impl(hubbard_model *m, const T *v0, int iters, double tau, double t, T *out_re, T *out_im, int *done,
+                           cudaStream_t st)
+{
+    std::vector<double> alpha((size_t)iters), beta((size_t)iters), yr((size_t)iters), yi((size_t)iters);
+    int n = 0;
+    int rc = lanczos_impl<T>(m, v0, iters, alpha.data(), beta.data(), &n, st);
+    if (rc) return rc;
+    if (done) *done = n;
+    if (n < 1) return HUBBARD_ERR_INVALID;
+    // |v0| (the run normalises its copy of v0 by a scalar; the propagated vector carries the norm)
+    const int64_t dim = model_dim(m);
+    const int vec_grid = lanczos_vec_grid(m, dim);
+    if ((rc = ensure_partials(m, vec_grid))) return rc;
+    vec_norm2_kernel<T><<<vec_grid, kVecThreads, 0, st>>>(v0, dim, m->d_scal, m->d_partial);
+    if ((rc = after_launch(m))) return rc;
+    LanczosScalars h{};
+    CU_TRY(m, cudaMemcpyAsync(&h, m->d_scal, sizeof(h), cudaMemcpyDeviceToHost, st));
+    CU_TRY(m, cudaStreamSynchronize(st));
+    const double nrm = std::sqrt(h.beta);
+    if ((rc = lanczos_expm_e1(alpha.data(), beta.data(), n, tau, t, yr.data(), yi.data()))) return rc;
+    for (int j = 0; j < n; ++j) { yr[(size_t)j] *= nrm; yi[(size_t)j] *= nrm; }
+    if ((rc = lanczos_combine<T>(m, v0, n, yr.data(), out_re, st))) return rc;
+    if (out_im && (rc = lanczos_combine<T>(m, v0, n, yi.data(), out_im, st))) return rc;
     return HUBBARD_OK;
 }
 
@@ -916,6 +955,23 @@ int lanczos_ground_state(hubbard_model *m, const void *v0_dev, int iters, void *
                                                 iters_done, st);
     return lanczos_ground_state_impl<double>(m, static_cast<const double *>(v0_dev), iters, static_cast<double *>(psi_dev), e0,
                                              iters_done, st);
+}
+
+int lanczos_propagate(hubbard_model *m, const void *v0_dev, int iters, double tau, double t, void *out_re_dev,
+                      void *out_im_dev, int *iters_done, void *stream)
+{
+    int rc = check_device_model(m);
+    if (rc) return rc;
+    if (iters_done) *iters_done = 0;
+    if (!v0_dev || !out_re_dev || iters < 1 || !std::isfinite(tau) || !std::isfinite(t)) return HUBBARD_ERR_INVALID;
+    if (v0_dev == out_re_dev || v0_dev == out_im_dev || out_re_dev == out_im_dev) return HUBBARD_ERR_INVALID;
+    if (((uintptr_t)v0_dev | (uintptr_t)out_re_dev | (uintptr_t)out_im_dev) & 15) return HUBBARD_ERR_INVALID;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (m->dtype == HUBBARD_F32)
+        return lanczos_propagate_impl<float>(m, static_cast<const float *>(v0_dev), iters, tau, t, static_cast<float *>(out_re_dev),
+                                             static_cast<float *>(out_im_dev), iters_done, st);
+    return lanczos_propagate_impl<double>(m, static_cast<const double *>(v0_dev), iters, tau, t, static_cast<double *>(out_re_dev),
+                                          static_cast<double *>(out_im_dev), iters_done, st);
 }
 
 int hubbard_apply_host(hubbard_model *m, const void *x_host, void *y_host, void *stream)

@@ -118,3 +118,89 @@ extern "C" int lanczos_ground_vector(const double *alpha, const double *beta, in
     delete[] piv;
     return HUBBARD_OK;
 }
+
+namespace {
+
+// All eigenvalues d[] and eigenvectors Z (row-major m x m, column k = vector k) of the symmetric tridiagonal
+// (d, e): implicit QL iteration with Wilkinson shifts (the classical EISPACK scheme restated), O(m^3) with the
+// eigenvector accumulation; m is at most a few hundred here.  e has m entries, e[m-1] unused.
+bool tridiag_eigh(int m, double *d, double *e, double *Z)
+{
+    for (int i = 0; i < m; ++i)
+        for (int k = 0; k < m; ++k) Z[(size_t)i * m + k] = (i == k) ? 1.0 : 0.0;
+    e[m - 1] = 0.0;
+    for (int l = 0; l < m; ++l) {
+        int iter = 0, mm;
+        do {
+            for (mm = l; mm < m - 1; ++mm) {
+                const double dd = std::fabs(d[mm]) + std::fabs(d[mm + 1]);
+                if (std::fabs(e[mm]) <= std::numeric_limits<double>::epsilon() * dd) break;
+            }
+            if (mm != l) {
+                if (iter++ == 200) return false;
+                double g = (d[l + 1] - d[l]) / (2.0 * e[l]);
+                double r = std::hypot(g, 1.0);
+                g = d[mm] - d[l] + e[l] / (g + (g >= 0.0 ? std::fabs(r) : -std::fabs(r)));
+                double s = 1.0, c = 1.0, p = 0.0;
+                int i;
+                for (i = mm - 1; i >= l; --i) {
+                    double f = s * e[i];
+                    const double b = c * e[i];
+                    r = std::hypot(f, g);
+                    e[i + 1] = r;
+                    if (r == 0.0) {
+                        d[i + 1] -= p;
+                        e[mm] = 0.0;
+                        break;
+                    }
+                    s = f / r;
+                    c = g / r;
+                    g = d[i + 1] - p;
+                    r = (d[i] - g) * s + 2.0 * c * b;
+                    p = s * r;
+                    d[i + 1] = g + p;
+                    g = c * r - b;
+                    for (int k = 0; k < m; ++k) {
+                        f = Z[(size_t)k * m + i + 1];
+                        Z[(size_t)k * m + i + 1] = s * Z[(size_t)k * m + i] + c * f;
+                        Z[(size_t)k * m + i] = c * Z[(size_t)k * m + i] - s * f;
+                    }
+                }
+                if (r == 0.0 && i >= l) continue;
+                d[l] -= p;
+                e[l] = g;
+                e[mm] = 0.0;
+            }
+        } while (mm != l);
+    }
+    return true;
+}
+
+}  // namespace
+
+// y = exp(-(tau + i t) T_m) e_1 (host utility for lanczos_propagate; "time propagation"):
+// T_m = Q diag(lambda) Q^T, y_j = sum_k Q[j][k] exp(-(tau + i t) lambda_k) Q[0][k].
+extern "C" int lanczos_expm_e1(const double *alpha, const double *beta, int m, double tau, double t, double *y_re,
+                               double *y_im)
+{
+    if (!alpha || m < 1 || (m > 1 && !beta) || !y_re || !y_im || !std::isfinite(tau) || !std::isfinite(t))
+        return HUBBARD_ERR_INVALID;
+    for (int i = 0; i < m; ++i)
+        if (!std::isfinite(alpha[i]) || (i + 1 < m && !std::isfinite(beta[i]))) return HUBBARD_ERR_INVALID;
+    double *buf = new (std::nothrow) double[(size_t)m * m + 2 * (size_t)m];
+    if (!buf) return HUBBARD_ERR_HOST_OOM;
+    double *Z = buf, *d = buf + (size_t)m * m, *e = d + m;
+    for (int i = 0; i < m; ++i) { d[i] = alpha[i]; e[i] = (i + 1 < m) ? beta[i] : 0.0; }
+    if (!tridiag_eigh(m, d, e, Z)) { delete[] buf; return HUBBARD_ERR_INVALID; }
+    for (int j = 0; j < m; ++j) y_re[j] = y_im[j] = 0.0;
+    for (int k = 0; k < m; ++k) {
+        const double w = std::exp(-tau * d[k]) * Z[k];            // Z[0][k]
+        const double cr = w * std::cos(t * d[k]), ci = -w * std::sin(t * d[k]);
+        for (int j = 0; j < m; ++j) {
+            y_re[j] += Z[(size_t)j * m + k] * cr;
+            y_im[j] += Z[(size_t)j * m + k] * ci;
+        }
+    }
+    delete[] buf;
+    return HUBBARD_OK;
+}

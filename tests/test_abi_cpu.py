@@ -212,3 +212,17 @@ def test_ground_vector_vs_lapack():
         assert np.max(np.abs(T @ y - e0 * y)) <= 1e-10 * max(1.0, np.max(np.abs(w)))
         if len(a) > 1 and w[1] - w[0] > 1e-6:
             assert abs(abs(np.dot(y, v[:, 0])) - 1.0) < 1e-8
+
+
+def test_expm_e1_vs_scipy():
+    """Host utility of lanczos_propagate: exp(-(tau + i t) T_m) e_1 against scipy's dense matrix exponential."""
+    from scipy.linalg import expm
+    rng = np.random.default_rng(11)
+    for m in (1, 2, 5, 60):
+        a = rng.normal(size=m) * 3
+        b = np.abs(rng.normal(size=max(m - 1, 0))) + 0.05
+        T = np.diag(a) + (np.diag(b, 1) + np.diag(b, -1) if m > 1 else 0)
+        for tau, t in ((0.0, 0.7), (0.4, 0.0), (0.2, -1.3)):
+            y = hb.lanczos_expm_e1(a, b, tau, t)
+            ref = expm(-(tau + 1j * t) * T)[:, 0]
+            assert np.max(np.abs(y - ref)) <= 1e-11 * max(1.0, np.max(np.abs(ref)))

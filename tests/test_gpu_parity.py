@@ -447,3 +447,54 @@ def test_lanczos_C4_prefix_vs_oracle(dtype):
     assert len(alpha) == n
     assert np.max(np.abs(alpha - a_ref) / np.maximum(1.0, np.abs(a_ref))) <= tol
     assert np.max(np.abs(beta - b_ref) / np.maximum(1.0, np.abs(b_ref))) <= tol
+
+
+# ---------------------------------------------------------------- SURVEY 8(f)-4
+@pytest.mark.parametrize("variant", ["paper", "twosweep", "gather", "persist"])
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_propagate_small_vs_dense_exponential(dtype, variant):
+    """lanczos_propagate against exp(-(tau + i t) H) v from the dense eigen-decomposition of the
+    definitional H (tier 0): real time, imaginary time and both; norm conservation in real time."""
+    ns, nu, nd, bonds, tt, U = 6, 3, 3, ring_bonds(6), 1.0, 4.0
+    H = hd.dense_hamiltonian(ns, nu, nd, bonds, tt, U)
+    w, Q = np.linalg.eigh(H)
+    m = hb.hubbard_create(ns, nu, nd, bonds, tt, U, dtype)
+    m.hubbard_set_variant(VARIANTS[variant])
+    v0, v0_np = start_vector(21, m.dim, dtype)
+    v0 *= 1.7                                           # the propagated vector must carry |v0|
+    v0_np = v0.double().cpu().numpy()
+    tol = 1e-9 if dtype == "f64" else 2e-4
+    for tau, t in ((0.0, 0.35), (0.25, 0.0), (0.1, -0.2)):
+        ref = Q @ (np.exp(-(tau + 1j * t) * w) * (Q.T @ v0_np))
+        re, im = torch.empty_like(v0), torch.empty_like(v0)
+        done = m.lanczos_propagate(v0, 60, tau, t, re, im)
+        assert done >= 1
+        got = re.double().cpu().numpy() + 1j * im.double().cpu().numpy()
+        assert np.max(np.abs(got - ref)) <= tol * np.max(np.abs(ref))
+        if tau == 0.0:
+            assert abs(np.linalg.norm(got) - np.linalg.norm(v0_np)) <= tol * np.linalg.norm(v0_np)
+    # imaginary part not requested
+    re2 = torch.empty_like(v0)
+    m.lanczos_propagate(v0, 60, 0.25, 0.0, re2, None)
+    ref = Q @ (np.exp(-0.25 * w) * (Q.T @ v0_np))
+    assert np.max(np.abs(re2.double().cpu().numpy() - ref)) <= tol * np.max(np.abs(ref))
+
+
+def test_propagate_C2_properties():
+    """C2 at full size (no dense exponential): unitarity in real time and agreement with the Taylor series of
+    exp(-i t H) v evaluated with the oracle's matrix-free H."""
+    c = CONFIGS["C2"]
+    m = hb.hubbard_create(c.n_sites, c.n_up, c.n_dn, c.bonds, c.t, 4.0, "f64")
+    ref = RefModel(c.n_sites, c.n_up, c.n_dn, c.bonds, c.t, 4.0)
+    v0, v0_np = start_vector(c.seed, c.dim, "f64")
+    re, im = torch.empty_like(v0), torch.empty_like(v0)
+    t = 0.05
+    m.lanczos_propagate(v0, 30, 0.0, t, re, im)
+    psi = re.double().cpu().numpy() + 1j * im.double().cpu().numpy()
+    assert abs(np.linalg.norm(psi) - 1.0) <= 1e-10
+    # Taylor series of exp(-i t H) v with the ORACLE's H*v (t |H| ~ 1.5: 30 terms are far past convergence)
+    term, acc = v0_np.astype(complex), v0_np.astype(complex)
+    for k in range(1, 31):
+        term = (-1j * t / k) * (ref.apply(term.real) + 1j * ref.apply(term.imag))
+        acc = acc + term
+    assert np.max(np.abs(psi - acc)) <= 1e-10 * np.max(np.abs(acc))
