@@ -232,7 +232,7 @@ int lanczos_expm_e1(const double *alpha, const double *beta, int m, double tau, 
  * bracketed by CUDA events on its stream; hubbard_kernel_times then returns,
  * per kernel class, the number of launches and the summed device time in ms
  * since the last hubbard_profile call (it synchronises the recorded events).
- * Classes: 0 = H v kernel(s) of variant PAPER, 1 = row sweep (down term),
+ * Classes: 0 = H v kernel(s) of variant PAPER and the cooperative kernel of PERSIST, 1 = row sweep (down term),
  * 2 = strip / column sweep (up term), 3 = Lanczos axpy+norm or closing norm
  * sweep, 4 = scalar/finalise kernels, 5 = setup (copy, initial norm).
  * Arrays have HUBBARD_N_KCLASS entries.
