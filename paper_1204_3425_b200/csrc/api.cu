@@ -5,6 +5,7 @@
 #include <cstring>
 #include <new>
 
+#include "kernels_cluster.cuh"
 #include "kernels_gather.cuh"
 #include "kernels_lanczos.cuh"
 #include "kernels_paper.cuh"
@@ -83,12 +84,39 @@ int gather_R_for(const hubbard_model *m)
     const size_t es = m->dtype == HUBBARD_F32 ? 4 : 8;
     const size_t budget = (size_t)std::max(0, m->max_smem_optin - 1024);
     const int64_t n_in = std::max(m->dn.dim, m->up.dim);
+    if (env_int("HUBBARD_FORCE_CLUSTER_ROW", 0)) return 0;      // tests: take the path of rows larger than one SM
     int forced = env_int("HUBBARD_GATHER_R", 0);
     for (int R = (int)(16 / es); R >= 1; R >>= 1) {
         if (forced > 0 && R > forced) continue;
         if ((size_t)(n_in + R + 128 / (R * es)) * R * es <= budget) return R;
     }
     return 0;
+}
+
+// A V row does not fit one SM but R rows fit the distributed shared memory of an NC-CTA cluster
+// (kernels_cluster.cuh).  Returns false if no (R, NC) does.
+bool cluster_row_config(const hubbard_model *m, int *R_out, int *NC_out, int *part_out)
+{
+    if (env_int("HUBBARD_NO_CLUSTER_ROW", 0) || m->dn.dim < 64) return false;
+    const int es = m->dtype == HUBBARD_F32 ? 4 : 8;
+    const int r_force = env_int("HUBBARD_CLUSTER_R", 0), nc_force = env_int("HUBBARD_CLUSTER_NC", 0);
+    // measured on C5 fp64: (R, NC) = (1, 2) 48.7 ms, (2, 4) 77.9 ms per sweep (the remote fraction and the 16-byte
+    // DSMEM loads dominate), single-SM L2 gathers 54.2 ms: the smallest cluster first, then the tallest tile
+    for (int NC : {2, 4}) {
+        if (nc_force && NC != nc_force) continue;
+        for (int R = 16 / es; R >= 1; R >>= 1) {
+            if (r_force && R != r_force) continue;
+            const int64_t part = ((m->dn.dim + NC - 1) / NC + 31) / 32 * 32;
+            const size_t need = (size_t)(part + 128 / (R * es)) * R * es;
+            if (need + 1024 <= (size_t)m->max_smem_optin && part * (NC - 1) < m->dn.dim) {
+                if (R_out) *R_out = R;
+                if (NC_out) *NC_out = NC;
+                if (part_out) *part_out = (int)part;
+                return true;
+            }
+        }
+    }
+    return false;
 }
 
 // Hop table of one spin for variant GATHER (kernels_gather.cuh, gather_tables.h).
@@ -166,6 +194,10 @@ int upload_tables(hubbard_model *m)
         if (m->gather_R > 0) {
             if ((rc = upload_gather_table(m, m->up, D.st_up, m->gather_R, &D.g_up))) return rc;
             if ((rc = upload_gather_table(m, m->dn, D.st_dn, m->gather_R, &D.g_dn))) return rc;
+        } else if (cluster_row_config(m, &m->cluster_R, &m->cluster_NC, &m->cluster_part)) {
+            // R rows fit the shared memory of a cluster: down-spin table in that layout for kernels_cluster.cuh
+            if ((rc = upload_gather_table(m, m->dn, D.st_dn, m->cluster_R, &D.g_dn))) return rc;
+            m->cluster_row = 1;
         }
     } catch (const std::bad_alloc &) {
         return HUBBARD_ERR_HOST_OOM;
@@ -432,6 +464,49 @@ int launch_strip(hubbard_model *m, SweepArgs<T> A, cudaStream_t st)
     return after_launch(m);
 }
 
+// Row half for rows larger than one SM's shared memory: clusters, the rows in distributed shared memory.
+template <typename T, typename E, int R, int NC>
+int launch_cluster_row_inst(hubbard_model *m, const ClusterRowArgs<T> &A, cudaStream_t st)
+{
+    auto kern = row_cluster_kernel<T, E, R, NC>;
+    const size_t smem = (size_t)(A.part + 128 / (R * sizeof(T))) * R * sizeof(T);
+    CU_TRY(m, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((unsigned)std::max(NC, m->sm_count / NC * NC));
+    cfg.blockDim = dim3(kClusterThreads);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr{};
+    attr.id = cudaLaunchAttributeClusterDimension;
+    attr.val.clusterDim.x = NC; attr.val.clusterDim.y = 1; attr.val.clusterDim.z = 1;
+    cfg.attrs = &attr;
+    cfg.numAttrs = 1;
+    ProfScope ps(m, 1, st);
+    CU_TRY(m, cudaLaunchKernelEx(&cfg, kern, A));
+    return after_launch(m);
+}
+
+template <typename T, typename E>
+int launch_cluster_row_e(hubbard_model *m, const ClusterRowArgs<T> &A, cudaStream_t st)
+{
+    const int R = m->cluster_R, NC = m->cluster_NC;
+    if constexpr (sizeof(T) == 4) {
+        if (R == 4) return NC == 2 ? launch_cluster_row_inst<T, E, 4, 2>(m, A, st) : launch_cluster_row_inst<T, E, 4, 4>(m, A, st);
+    }
+    if (R == 2) return NC == 2 ? launch_cluster_row_inst<T, E, 2, 2>(m, A, st) : launch_cluster_row_inst<T, E, 2, 4>(m, A, st);
+    return NC == 2 ? launch_cluster_row_inst<T, E, 1, 2>(m, A, st) : launch_cluster_row_inst<T, E, 1, 4>(m, A, st);
+}
+
+template <typename T>
+int launch_cluster_row(hubbard_model *m, const T *x, T *y, LanczosScalars *S, cudaStream_t st)
+{
+    ClusterRowArgs<T> A{};
+    A.in = m->dev.g_dn; A.st_up = m->dev.st_up; A.dim_up = m->dev.dim_up; A.dim_dn = m->dev.dim_dn;
+    A.part = m->cluster_part;
+    A.t = m->t; A.U = m->U; A.x = x; A.y = y; A.S = S;
+    return A.in.e16 ? launch_cluster_row_e<T, uint16_t>(m, A, st) : launch_cluster_row_e<T, uint32_t>(m, A, st);
+}
+
 // y = H x (LZ = false) or the fused Lanczos H f_j - b_j f_{j-1}, a_j (LZ = true)
 template <typename T, bool LZ>
 int apply_impl(hubbard_model *m, const T *x, T *y, cudaStream_t st)
@@ -470,6 +545,8 @@ int apply_impl(hubbard_model *m, const T *x, T *y, cudaStream_t st)
         GatherArgs<T> G{};
         G.x = x; G.y = y; G.y_rowmajor = 1; G.S = LZ ? m->d_scal : nullptr;
         rc = launch_gather<T, false, false>(m, G, st);
+    } else if (m->variant == HUBBARD_VARIANT_AUTO && m->cluster_row) {
+        rc = launch_cluster_row<T>(m, x, y, LZ ? m->d_scal : nullptr, st);
     } else {
         rc = m->dev.dn_ent16 ? launch_row<T, uint16_t, LZ>(m, A, m->dev.dn_ent16, st)
                              : launch_row<T, uint32_t, LZ>(m, A, m->dev.dn_ent32, st);

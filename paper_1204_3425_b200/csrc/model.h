@@ -82,6 +82,8 @@ struct hubbard_model {
     int sm_count = 148;
     int max_smem_optin = 0;
     int coop_launch = 0;               // device supports cooperative launches (variant PERSIST)
+    int cluster_row = 0;               // rows go through clusters (kernels_cluster.cuh): gather_R == 0 but a cluster holds them
+    int cluster_R = 0, cluster_NC = 0, cluster_part = 0;
     int gather_R = 0;                  // tile height of variant GATHER, 0 = does not fit
 
     hub::DevModel dev{};

@@ -498,3 +498,30 @@ def test_propagate_C2_properties():
         term = (-1j * t / k) * (ref.apply(term.real) + 1j * ref.apply(term.imag))
         acc = acc + term
     assert np.max(np.abs(psi - acc)) <= 1e-10 * np.max(np.abs(acc))
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("R,NC", [(0, 0), (1, 2), (1, 4), (2, 2), (2, 4)])
+@pytest.mark.parametrize("name,ns,nu,nd,bonds", [("C2", 12, 6, 6, ring_bonds(12)), ("odd", 13, 5, 7, ring_bonds(13) + [(0, 5)])])
+def test_cluster_row_sweep(name, ns, nu, nd, bonds, R, NC, dtype, monkeypatch):
+    """The distributed-shared-memory row sweep (clusters of NC CTAs holding R rows, kernels_cluster.cuh: what
+    C5 fp64 uses because a V row exceeds one SM) forced on sectors the oracle covers in full: H*v and a Lanczos
+    run; dim_dn not a multiple of 32 or of the cluster split, N_up != N_dn, odd dim_up with R = 2."""
+    monkeypatch.setenv("HUBBARD_FORCE_CLUSTER_ROW", "1")
+    monkeypatch.setenv("HUBBARD_CLUSTER_R", str(R))
+    monkeypatch.setenv("HUBBARD_CLUSTER_NC", str(NC))
+    ref = RefModel(ns, nu, nd, bonds, 1.0, 4.0)
+    m = hb.hubbard_create(ns, nu, nd, bonds, 1.0, 4.0, dtype)
+    x, x_np = start_vector(77, m.dim, dtype)
+    y = torch.full_like(x, float("nan"))
+    m.hubbard_apply(x, y)
+    torch.cuda.synchronize()
+    assert rel_max_err(y, ref.apply(x_np)) <= TOL_HV[dtype]
+    assert m.hubbard_kernel_times is not None
+    m.hubbard_profile(True)
+    alpha, beta = m.lanczos_run(x, 40)
+    assert m.hubbard_kernel_times()["row_sweep"][0] == 40          # the cluster kernel is the row sweep of every iteration
+    m.hubbard_profile(False)
+    a_ref, b_ref = lr.lanczos(ref.apply, x_np, 40)
+    e_ref = lr.ground_energy(a_ref, b_ref)
+    assert abs(hb.lanczos_ground_energy(alpha, beta) - e_ref) <= TOL_E0[dtype] * abs(e_ref)
