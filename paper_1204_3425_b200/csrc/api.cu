@@ -545,7 +545,8 @@ int apply_impl(hubbard_model *m, const T *x, T *y, cudaStream_t st)
         GatherArgs<T> G{};
         G.x = x; G.y = y; G.y_rowmajor = 1; G.S = LZ ? m->d_scal : nullptr;
         rc = launch_gather<T, false, false>(m, G, st);
-    } else if (m->variant == HUBBARD_VARIANT_AUTO && m->cluster_row) {
+    } else if (m->variant == HUBBARD_VARIANT_AUTO && m->cluster_row && (LZ || env_int("HUBBARD_FORCE_CLUSTER_ROW", 0))) {
+        // (plain apply, which reads no y, is faster through the single-SM L2 gathers: 39.6 vs 47 ms on C5 fp64)
         rc = launch_cluster_row<T>(m, x, y, LZ ? m->d_scal : nullptr, st);
     } else {
         rc = m->dev.dn_ent16 ? launch_row<T, uint16_t, LZ>(m, A, m->dev.dn_ent16, st)
