@@ -59,7 +59,8 @@ enum {
  * variant computes the same H v). */
 enum {
     HUBBARD_VARIANT_AUTO = 0,    /* library picks per model (default) */
-    HUBBARD_VARIANT_PAPER = 1,   /* Algorithms 2-4 restated: one thread per element, one fused kernel */
+    HUBBARD_VARIANT_PAPER = 1,   /* Algorithms 2-4 restated: one thread per element, one fused kernel (or four
+                                    sub-vectors per block: hubbard_debug_set "paper_subvectors") */
     HUBBARD_VARIANT_TWOSWEEP = 2,/* row sweep (down term + diagonal, row staged in shared memory)
                                     + strip sweep (up term over L2-resident column strips) */
     HUBBARD_VARIANT_GATHER = 3,  /* symmetric gather sweeps: R whole rows (down term) then R whole
@@ -241,6 +242,27 @@ int lanczos_expm_e1(const double *alpha, const double *beta, int m, double tau, 
 int hubbard_profile(hubbard_model *m, int enable);
 int hubbard_kernel_times(hubbard_model *m, int64_t *launches, double *ms);
 int64_t hubbard_launch_count(const hubbard_model *m);
+
+/* ---- development / test knobs (per model; nothing is read from the environment) ----
+ * hubbard_debug_set forces one dispatch or geometry decision of this model so that a test or an A/B measurement
+ * states what it forces; the defaults are what bench.py times and what production callers get.  Keys (value range):
+ *   "gather_R" (0-4)          cap on the tile height R of variant GATHER, 0 = none (what a larger sector would get)
+ *   "gather_nosched" (0/1)    hop entries in bond order, no bank-aware placement
+ *   "gather_ctas" (1-4)       CTAs per SM for small tiles
+ *   "apply_pure_gather" (0/1) plain hubbard_apply as two gather sweeps instead of the hybrid
+ *   "twosweep_old_row" (0/1)  AUTO's TWOSWEEP fallback keeps the first row kernel
+ *   "row_R" (0-4), "strip_mb" (1-1024), "strip_rb"   geometry of variant TWOSWEEP (0 = automatic)
+ *   "persist_max_dim"         largest dim that AUTO runs in the cooperative kernel
+ *   "paper_subvectors" (1 or 4)  variant PAPER: sub-vectors per block = elements per thread (4 = the paper's tuned
+ *                             form; any other value means 1)
+ *   "force_cluster_row" (0/1), "no_cluster_row" (0/1), "cluster_R" (0-4), "cluster_NC" (0,2,4)
+ *                             take / avoid the cluster row sweep of rows larger than one SM, force one (R, NC)
+ * Options that change a device table layout re-upload that table (host work + cudaMemcpy; no kernel launch).
+ * hubbard_debug_get returns an option, or what the library resolved for this model: "resolved_variant"
+ * (HUBBARD_VARIANT_* that AUTO stands for), "resolved_gather_R", "resolved_cluster_row", "resolved_cluster_R",
+ * "resolved_cluster_NC".  Unknown key or out-of-range value: HUBBARD_ERR_INVALID. */
+int hubbard_debug_set(hubbard_model *m, const char *key, int value);
+int hubbard_debug_get(const hubbard_model *m, const char *key, int *value);
 
 /* Last CUDA error code (cudaError_t as int) seen by this model, 0 if none. */
 int hubbard_last_cuda_error(const hubbard_model *m);

@@ -23,7 +23,7 @@ ABI_SYMBOLS = (
     "lanczos_ground_vector", "lanczos_propagate", "lanczos_expm_e1", "lanczos_set_tau", "hubbard_apply_host",
     "lanczos_run_host", "hubbard_get_basis", "hubbard_get_hops", "hubbard_get_gather_table", "lanczos_ground_energy",
     "hubbard_profile", "hubbard_kernel_times", "hubbard_launch_count", "hubbard_last_cuda_error",
-    "hubbard_strerror",
+    "hubbard_strerror", "hubbard_debug_set", "hubbard_debug_get",
 )
 
 
@@ -63,6 +63,8 @@ def _load() -> C.CDLL:
     lib.hubbard_launch_count.argtypes = [vp]
     lib.hubbard_launch_count.restype = i64
     lib.hubbard_last_cuda_error.argtypes = [vp]
+    lib.hubbard_debug_set.argtypes = [vp, C.c_char_p, i32]
+    lib.hubbard_debug_get.argtypes = [vp, C.c_char_p, P(i32)]
     lib.hubbard_strerror.argtypes = [i32]
     lib.hubbard_strerror.restype = C.c_char_p
     return lib
@@ -152,6 +154,14 @@ class Model:
 
     def lanczos_set_tau(self, tau):
         _check(lib.lanczos_set_tau(self._h, float(tau)), "lanczos_set_tau")
+
+    def hubbard_debug_set(self, key, value):
+        _check(lib.hubbard_debug_set(self._h, key.encode(), int(value)), f"hubbard_debug_set({key})", self._h)
+
+    def hubbard_debug_get(self, key):
+        v = C.c_int(0)
+        _check(lib.hubbard_debug_get(self._h, key.encode(), C.byref(v)), f"hubbard_debug_get({key})")
+        return v.value
 
     # -- hot path, device buffers (torch CUDA tensors)
     def hubbard_apply(self, x, y, stream=None):

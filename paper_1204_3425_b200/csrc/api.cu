@@ -3,7 +3,9 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
+#include <unordered_map>
 
 #include "kernels_cluster.cuh"
 #include "kernels_gather.cuh"
@@ -28,13 +30,14 @@ namespace {
         }                                                                 \
     } while (0)
 
+// `layout` = the table depends on the model's DebugOptions and is rebuilt when they change
 template <typename U>
-int dev_upload(hubbard_model *m, const std::vector<U> &h, const U **out)
+int dev_upload(hubbard_model *m, const std::vector<U> &h, const U **out, bool layout = false)
 {
     void *p = nullptr;
     size_t bytes = std::max<size_t>(h.size(), 1) * sizeof(U);
     CU_TRY(m, cudaMalloc(&p, bytes));
-    m->dev_allocs.push_back(p);
+    (layout ? m->layout_allocs : m->dev_allocs).push_back(p);
     if (!h.empty()) CU_TRY(m, cudaMemcpy(p, h.data(), h.size() * sizeof(U), cudaMemcpyHostToDevice));
     *out = static_cast<const U *>(p);
     return HUBBARD_OK;
@@ -69,13 +72,6 @@ int build_host(hubbard_model **out, int n_sites, int n_up, int n_dn, const int32
     return HUBBARD_OK;
 }
 
-int env_int(const char *name, int dflt)
-{
-    const char *v = getenv(name);
-    if (!v || !*v) return dflt;
-    return atoi(v);
-}
-
 // Tile height R (rows per ROW tile = columns per COL tile) of variant GATHER:
 // the largest R with R * sizeof(T) <= 16 for which a whole row AND a whole
 // column of V fit in shared memory; 0 if even R = 1 does not fit.
@@ -84,8 +80,8 @@ int gather_R_for(const hubbard_model *m)
     const size_t es = m->dtype == HUBBARD_F32 ? 4 : 8;
     const size_t budget = (size_t)std::max(0, m->max_smem_optin - 1024);
     const int64_t n_in = std::max(m->dn.dim, m->up.dim);
-    if (env_int("HUBBARD_FORCE_CLUSTER_ROW", 0)) return 0;      // tests: take the path of rows larger than one SM
-    int forced = env_int("HUBBARD_GATHER_R", 0);
+    if (m->opt.force_cluster_row) return 0;                     // tests: take the path of rows larger than one SM
+    const int forced = m->opt.gather_R;
     for (int R = (int)(16 / es); R >= 1; R >>= 1) {
         if (forced > 0 && R > forced) continue;
         if ((size_t)(n_in + R + 128 / (R * es)) * R * es <= budget) return R;
@@ -97,9 +93,9 @@ int gather_R_for(const hubbard_model *m)
 // (kernels_cluster.cuh).  Returns false if no (R, NC) does.
 bool cluster_row_config(const hubbard_model *m, int *R_out, int *NC_out, int *part_out)
 {
-    if (env_int("HUBBARD_NO_CLUSTER_ROW", 0) || m->dn.dim < 64) return false;
+    if (m->opt.no_cluster_row || m->dn.dim < 64) return false;
     const int es = m->dtype == HUBBARD_F32 ? 4 : 8;
-    const int r_force = env_int("HUBBARD_CLUSTER_R", 0), nc_force = env_int("HUBBARD_CLUSTER_NC", 0);
+    const int r_force = m->opt.cluster_R, nc_force = m->opt.cluster_NC;
     // measured on C5 fp64: (R, NC) = (1, 2) 48.7 ms, (2, 4) 77.9 ms per sweep (the remote fraction and the 16-byte
     // DSMEM loads dominate), single-SM L2 gathers 54.2 ms: the smallest cluster first, then the tallest tile
     for (int NC : {2, 4}) {
@@ -126,21 +122,48 @@ int upload_gather_table(hubbard_model *m, const SpinTable &tab, const uint32_t *
     G.dim = tab.dim;
     G.st = d_states;
     const int es = m->dtype == HUBBARD_F32 ? 4 : 8;
-    const int lanes = env_int("HUBBARD_GATHER_NOSCHED", 0) ? 0 : 128 / (R * es);
+    const int lanes = m->opt.gather_nosched ? 0 : 128 / (R * es);
     GatherTable T;
     build_gather_table(tab, lanes, (tab.dim + R - 1) / R * R, T);
     G.w = T.w;
     G.ld = T.ld;
     int rc;
-    if ((rc = dev_upload(m, T.ent, &G.e32))) return rc;
-    if ((rc = dev_upload(m, T.cnt, &G.cnt))) return rc;
+    if ((rc = dev_upload(m, T.ent, &G.e32, true))) return rc;
+    if ((rc = dev_upload(m, T.cnt, &G.cnt, true))) return rc;
     G.e16 = nullptr;
     if (tab.dim + 1 + 128 <= 32768) {
         std::vector<uint16_t> e16(T.ent.size());
         for (size_t i = 0; i < T.ent.size(); ++i) e16[i] = (uint16_t)T.ent[i];
-        if ((rc = dev_upload(m, e16, &G.e16))) return rc;
+        if ((rc = dev_upload(m, e16, &G.e16, true))) return rc;
     }
     *out = G;
+    return HUBBARD_OK;
+}
+
+// The tables whose layout depends on the model's DebugOptions (tile height of variant GATHER, cluster row
+// configuration); called by hubbard_create and again by hubbard_debug_set when such an option changes.
+int upload_layout_tables(hubbard_model *m)
+{
+    DevModel &D = m->dev;
+    for (void *p : m->layout_allocs) cudaFree(p);
+    m->layout_allocs.clear();
+    D.g_up = SpinDev{}; D.g_dn = SpinDev{};
+    m->cluster_row = 0; m->cluster_R = m->cluster_NC = m->cluster_part = 0;
+    int rc;
+    try {
+        // variant GATHER: both spins column-major, entry = col * 2 + neg
+        m->gather_R = gather_R_for(m);
+        if (m->gather_R > 0) {
+            if ((rc = upload_gather_table(m, m->up, D.st_up, m->gather_R, &D.g_up))) return rc;
+            if ((rc = upload_gather_table(m, m->dn, D.st_dn, m->gather_R, &D.g_dn))) return rc;
+        } else if (cluster_row_config(m, &m->cluster_R, &m->cluster_NC, &m->cluster_part)) {
+            // R rows fit the shared memory of a cluster: down-spin table in that layout for kernels_cluster.cuh
+            if ((rc = upload_gather_table(m, m->dn, D.st_dn, m->cluster_R, &D.g_dn))) return rc;
+            m->cluster_row = 1;
+        }
+    } catch (const std::bad_alloc &) {
+        return HUBBARD_ERR_HOST_OOM;
+    }
     return HUBBARD_OK;
 }
 
@@ -189,26 +212,23 @@ int upload_tables(hubbard_model *m)
             for (size_t i = 0; i < de.size(); ++i) d16[i] = (uint16_t)de[i];
             if ((rc = dev_upload(m, d16, &D.dn_ent16))) return rc;
         }
-        // variant GATHER: both spins column-major, entry = col * 2 + neg
-        m->gather_R = gather_R_for(m);
-        if (m->gather_R > 0) {
-            if ((rc = upload_gather_table(m, m->up, D.st_up, m->gather_R, &D.g_up))) return rc;
-            if ((rc = upload_gather_table(m, m->dn, D.st_dn, m->gather_R, &D.g_dn))) return rc;
-        } else if (cluster_row_config(m, &m->cluster_R, &m->cluster_NC, &m->cluster_part)) {
-            // R rows fit the shared memory of a cluster: down-spin table in that layout for kernels_cluster.cuh
-            if ((rc = upload_gather_table(m, m->dn, D.st_dn, m->cluster_R, &D.g_dn))) return rc;
-            m->cluster_row = 1;
-        }
     } catch (const std::bad_alloc &) {
         return HUBBARD_ERR_HOST_OOM;
     }
-    return HUBBARD_OK;
+    return upload_layout_tables(m);
 }
 
 }  // namespace
 
 // ------------------------------------------------------------------ launches
 namespace {
+
+// Events come from a per-model pool (created once, reused): no cudaEventCreate inside a timed region after warm-up.
+bool pool_event(hubbard_model *m, cudaEvent_t *e)
+{
+    if (!m->event_pool.empty()) { *e = m->event_pool.back(); m->event_pool.pop_back(); return true; }
+    return cudaEventCreate(e) == cudaSuccess;
+}
 
 struct ProfScope {
     hubbard_model *m;
@@ -219,7 +239,8 @@ struct ProfScope {
     {
         if (!on) return;
         rec.kclass = kclass;
-        if (cudaEventCreate(&rec.e0) != cudaSuccess || cudaEventCreate(&rec.e1) != cudaSuccess) { on = false; return; }
+        if (!pool_event(m, &rec.e0)) { on = false; return; }
+        if (!pool_event(m, &rec.e1)) { m->event_pool.push_back(rec.e0); on = false; return; }
         cudaEventRecord(rec.e0, st);
     }
     ~ProfScope()
@@ -229,6 +250,22 @@ struct ProfScope {
         m->prof.push_back(rec);
     }
 };
+
+// cudaFuncSetAttribute(MaxDynamicSharedMemorySize) is per function and process-wide: it is raised at most once
+// per (kernel, size) and never lowered, so the launch path of a warmed-up model makes no attribute call.
+template <typename K>
+int ensure_smem(hubbard_model *m, K kern, size_t smem, bool carveout = false)
+{
+    static std::mutex mu;
+    static std::unordered_map<const void *, size_t> granted;
+    std::lock_guard<std::mutex> lock(mu);
+    size_t &cur = granted[(const void *)kern];
+    if (cur >= smem && cur > 0) return HUBBARD_OK;
+    CU_TRY(m, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    if (carveout) CU_TRY(m, cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
+    cur = smem;
+    return HUBBARD_OK;
+}
 
 int after_launch(hubbard_model *m)
 {
@@ -270,7 +307,7 @@ int resolve_variant(const hubbard_model *m)
     if (m->variant != HUBBARD_VARIANT_AUTO) return m->variant;
     // very small sectors (C1): the Lanczos loop is launch-latency bound -> one cooperative kernel (measured: C1 10.8 vs
     // 17.2 us per iteration; already C2, 854 k elements, is faster with the gather sweeps: 31.8 vs 39.3 us)
-    if (m->up.dim * m->dn.dim <= (int64_t)env_int("HUBBARD_PERSIST_MAX_DIM", 1 << 17) && m->coop_launch) return HUBBARD_VARIANT_PERSIST;
+    if (m->up.dim * m->dn.dim <= (int64_t)m->opt.persist_max_dim && m->coop_launch) return HUBBARD_VARIANT_PERSIST;
     if (m->dn.dim < 512 || m->up.dim < 512) return HUBBARD_VARIANT_PAPER;
     // GATHER pays off when the R x R blocks it writes transposed are whole sectors (R * sizeof(T) = 16);
     // with a narrower tile (C5 fp32: R = 1) its strided writes are 4-byte pieces and TWOSWEEP is faster.
@@ -290,13 +327,12 @@ int launch_gather_inst(hubbard_model *m, GatherArgs<T> A, cudaStream_t st)
     const size_t cnt_bytes = (size_t)round_up(n_in_p, 32);
     A.cnt_in_smem = (A.in.w < 256 && smem + cnt_bytes + 1024 <= (size_t)m->max_smem_optin) ? 1 : 0;
     if (A.cnt_in_smem) smem += cnt_bytes;
-    CU_TRY(m, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    CU_TRY(m, cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
+    if (int rc = ensure_smem(m, kern, smem, true)) return rc;
     const int64_t tiles = (COL ? A.dd_p : A.du_p) / R;
     // Small sectors: several CTAs per SM (their staging and gather phases overlap one another); the 64-register
     // kernels allow 1024 threads per SM in total.
     int per_sm = (int)std::min<size_t>(4, (size_t)(m->max_smem_optin - 2048) / (smem + 1024));
-    per_sm = std::max(1, std::min(per_sm, env_int("HUBBARD_GATHER_CTAS", 4)));
+    per_sm = std::max(1, std::min(per_sm, m->opt.gather_ctas));
     const int threads = std::max(32, kGatherMaxThreads / per_sm / 32 * 32);
     const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(tiles, (int64_t)m->sm_count * per_sm));
     {
@@ -375,14 +411,18 @@ template <typename T, bool LZ>
 int launch_paper(hubbard_model *m, const T *x, T *y, cudaStream_t st)
 {
     const DevModel &D = m->dev;
+    const int sub = m->opt.paper_subvectors == 4 ? 4 : 1;
     int64_t bps = (D.dim_dn + kPaperThreads - 1) / kPaperThreads;
-    int64_t gy = std::min<int64_t>(D.dim_up, 65535);
+    int64_t gy = std::min<int64_t>((D.dim_up + sub - 1) / sub, 65535);
     if (LZ) gy = std::max<int64_t>(1, std::min<int64_t>(gy, (1 << 16) / bps));
     if (bps > 0x7fffffff) return HUBBARD_ERR_UNSUPPORTED;
     SweepArgs<T> A{x, y, LZ ? m->d_scal : nullptr, m->d_partial};
     if (LZ) { int rc = ensure_partials(m, bps * gy); if (rc) return rc; A.partials = m->d_partial; }
     ProfScope ps(m, 0, st);
-    hv_paper_kernel<T, LZ><<<dim3((unsigned)bps, (unsigned)gy), kPaperThreads, (size_t)D.w_up * 4, st>>>(D, A);
+    const dim3 grid((unsigned)bps, (unsigned)gy);
+    const size_t smem = (size_t)sub * D.w_up * 4;
+    if (sub == 4) hv_paper_kernel<T, LZ, 4><<<grid, kPaperThreads, smem, st>>>(D, A);
+    else hv_paper_kernel<T, LZ, 1><<<grid, kPaperThreads, smem, st>>>(D, A);
     return after_launch(m);
 }
 
@@ -391,7 +431,7 @@ template <typename T, typename E, int R, bool LZ>
 int launch_row_staged(hubbard_model *m, const SweepArgs<T> &A, const E *ent, size_t smem, cudaStream_t st)
 {
     auto kern = row_sweep_kernel<T, E, R, LZ>;
-    CU_TRY(m, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    if (int rc = ensure_smem(m, kern, smem)) return rc;
     int per_sm = std::max(1, std::min(2, (int)((size_t)m->max_smem_optin / (smem + 1024))));
     int64_t groups = (m->dev.dim_up + R - 1) / R;
     int grid = (int)std::min<int64_t>(groups, (int64_t)m->sm_count * per_sm);
@@ -406,7 +446,7 @@ int launch_row(hubbard_model *m, const SweepArgs<T> &A, const E *ent, cudaStream
     const DevModel &D = m->dev;
     constexpr int N = 16 / sizeof(T);
     auto need = [&](int R) { return ((size_t)R * D.dim_dn + N) * sizeof(T); };
-    int R = env_int("HUBBARD_ROW_R", 0);
+    int R = m->opt.row_R;
     if (R == 0) {
         // default: the largest R in {4,2,1} that still lets two CTAs share an SM, else R = 1
         R = 1;
@@ -437,14 +477,14 @@ int launch_strip(hubbard_model *m, SweepArgs<T> A, cudaStream_t st)
     int VW = N;
     while (VW > 1 && (D.dim_dn % VW) != 0) VW >>= 1;
     StripPlan P;
-    double mb = (double)env_int("HUBBARD_STRIP_MB", 24);
+    double mb = (double)m->opt.strip_mb;
     int64_t W = (int64_t)(mb * 1048576.0 / ((double)D.dim_up * sizeof(T)));
     W = std::max<int64_t>(32, W / 32 * 32);
     int64_t dd_up = (D.dim_dn + VW - 1) / VW * VW;
     W = std::min(W, dd_up);
     P.W = W;
     P.n_strips = (D.dim_dn + W - 1) / W;
-    int RB = env_int("HUBBARD_STRIP_RB", 0);
+    int RB = m->opt.strip_rb;
     if (RB <= 0) RB = (int)std::max<int64_t>(8, (2048 * (int64_t)VW + W - 1) / W);
     RB = (int)std::min<int64_t>(RB, D.dim_up);
     P.RB = RB;
@@ -470,7 +510,7 @@ int launch_cluster_row_inst(hubbard_model *m, const ClusterRowArgs<T> &A, cudaSt
 {
     auto kern = row_cluster_kernel<T, E, R, NC>;
     const size_t smem = (size_t)(A.part + 128 / (R * sizeof(T))) * R * sizeof(T);
-    CU_TRY(m, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    if (int rc = ensure_smem(m, kern, smem)) return rc;
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3((unsigned)std::max(NC, m->sm_count / NC * NC));
     cfg.blockDim = dim3(kClusterThreads);
@@ -517,7 +557,7 @@ int apply_impl(hubbard_model *m, const T *x, T *y, cudaStream_t st)
     if (variant == HUBBARD_VARIANT_PAPER || variant == HUBBARD_VARIANT_PERSIST) return launch_paper<T, LZ>(m, x, y, st);
     if (variant == HUBBARD_VARIANT_GATHER) {
         if (LZ) return HUBBARD_ERR_INVALID;          // the Lanczos form of GATHER is lanczos_gather_impl
-        if (m->variant == HUBBARD_VARIANT_AUTO && !env_int("HUBBARD_APPLY_PURE_GATHER", 0)) {
+        if (m->variant == HUBBARD_VARIANT_AUTO && !m->opt.apply_pure_gather) {
             // plain y = H x on row-major vectors: gather ROW sweep (down term + diagonal, written row-major, no
             // intermediate layouts) followed by the strip sweep of TWOSWEEP (up term over L2-resident strips):
             // measured 4.0 ms against 5.0 ms for either pure form on C4 fp64
@@ -539,13 +579,13 @@ int apply_impl(hubbard_model *m, const T *x, T *y, cudaStream_t st)
     }
     SweepArgs<T> A{x, y, LZ ? m->d_scal : nullptr, m->d_partial};
     int rc;
-    if (m->variant == HUBBARD_VARIANT_AUTO && gather_R(m) > 0 && !env_int("HUBBARD_TWOSWEEP_OLD_ROW", 0)) {
+    if (m->variant == HUBBARD_VARIANT_AUTO && gather_R(m) > 0 && !m->opt.twosweep_old_row) {
         // AUTO fell back to TWOSWEEP because the tile is narrower than 16 bytes (C5 fp32): the row half still runs
         // as the gather ROW sweep on row-major vectors (batch-interleaved, bank-aware tables; vectorised staging)
         GatherArgs<T> G{};
         G.x = x; G.y = y; G.y_rowmajor = 1; G.S = LZ ? m->d_scal : nullptr;
         rc = launch_gather<T, false, false>(m, G, st);
-    } else if (m->variant == HUBBARD_VARIANT_AUTO && m->cluster_row && (LZ || env_int("HUBBARD_FORCE_CLUSTER_ROW", 0))) {
+    } else if (m->variant == HUBBARD_VARIANT_AUTO && m->cluster_row && (LZ || m->opt.force_cluster_row)) {
         // (plain apply, which reads no y, is faster through the single-SM L2 gathers: 39.6 vs 47 ms on C5 fp64)
         rc = launch_cluster_row<T>(m, x, y, LZ ? m->d_scal : nullptr, st);
     } else {
@@ -934,7 +974,9 @@ void hubbard_destroy(hubbard_model *m)
 {
     if (!m) return;
     for (auto &r : m->prof) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
+    for (cudaEvent_t e : m->event_pool) cudaEventDestroy(e);
     for (void *p : m->dev_allocs) cudaFree(p);
+    for (void *p : m->layout_allocs) cudaFree(p);
     for (int i = 0; i < 6; ++i) if (m->work[i]) cudaFree(m->work[i]);
     if (m->d_ycoef) cudaFree(m->d_ycoef);
     for (int i = 0; i < 2; ++i) if (m->stage[i]) cudaFree(m->stage[i]);
@@ -1119,10 +1161,63 @@ int hubbard_get_gather_table(const hubbard_model *m, int spin, int lanes, int64_
     return HUBBARD_OK;
 }
 
+// ---- development / test knobs (DebugOptions, model.h)
+namespace {
+struct OptKey { const char *name; int hub::DebugOptions::*field; bool layout; int lo, hi; };
+const OptKey kOptKeys[] = {
+    {"gather_R", &hub::DebugOptions::gather_R, true, 0, 4},
+    {"gather_nosched", &hub::DebugOptions::gather_nosched, true, 0, 1},
+    {"gather_ctas", &hub::DebugOptions::gather_ctas, false, 1, 4},
+    {"apply_pure_gather", &hub::DebugOptions::apply_pure_gather, false, 0, 1},
+    {"twosweep_old_row", &hub::DebugOptions::twosweep_old_row, false, 0, 1},
+    {"row_R", &hub::DebugOptions::row_R, false, 0, 4},
+    {"strip_mb", &hub::DebugOptions::strip_mb, false, 1, 1024},
+    {"strip_rb", &hub::DebugOptions::strip_rb, false, 0, 1 << 20},
+    {"persist_max_dim", &hub::DebugOptions::persist_max_dim, false, 0, 1 << 30},
+    {"force_cluster_row", &hub::DebugOptions::force_cluster_row, true, 0, 1},
+    {"no_cluster_row", &hub::DebugOptions::no_cluster_row, true, 0, 1},
+    {"cluster_R", &hub::DebugOptions::cluster_R, true, 0, 4},
+    {"cluster_NC", &hub::DebugOptions::cluster_NC, true, 0, 4},
+    {"paper_subvectors", &hub::DebugOptions::paper_subvectors, false, 1, 4},
+};
+}  // namespace
+
+int hubbard_debug_set(hubbard_model *m, const char *key, int value)
+{
+    if (!m || !key) return HUBBARD_ERR_INVALID;
+    for (const OptKey &k : kOptKeys) {
+        if (std::strcmp(key, k.name) != 0) continue;
+        if (value < k.lo || value > k.hi) return HUBBARD_ERR_INVALID;
+        if (m->opt.*(k.field) == value) return HUBBARD_OK;
+        m->opt.*(k.field) = value;
+        if (k.layout && m->has_device) {
+            const int rc = upload_layout_tables(m);
+            if (rc) return rc;
+            if (m->variant == HUBBARD_VARIANT_GATHER && !gather_fits(m)) m->variant = HUBBARD_VARIANT_AUTO;
+        }
+        return HUBBARD_OK;
+    }
+    return HUBBARD_ERR_INVALID;
+}
+
+int hubbard_debug_get(const hubbard_model *m, const char *key, int *value)
+{
+    if (!m || !key || !value) return HUBBARD_ERR_INVALID;
+    for (const OptKey &k : kOptKeys)
+        if (std::strcmp(key, k.name) == 0) { *value = m->opt.*(k.field); return HUBBARD_OK; }
+    // what the library resolved (read-only)
+    if (!std::strcmp(key, "resolved_variant")) { *value = m->has_device ? resolve_variant(m) : m->variant; return HUBBARD_OK; }
+    if (!std::strcmp(key, "resolved_gather_R")) { *value = m->gather_R; return HUBBARD_OK; }
+    if (!std::strcmp(key, "resolved_cluster_row")) { *value = m->cluster_row; return HUBBARD_OK; }
+    if (!std::strcmp(key, "resolved_cluster_R")) { *value = m->cluster_R; return HUBBARD_OK; }
+    if (!std::strcmp(key, "resolved_cluster_NC")) { *value = m->cluster_NC; return HUBBARD_OK; }
+    return HUBBARD_ERR_INVALID;
+}
+
 int hubbard_profile(hubbard_model *m, int enable)
 {
     if (!m) return HUBBARD_ERR_INVALID;
-    for (auto &r : m->prof) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
+    for (auto &r : m->prof) { m->event_pool.push_back(r.e0); m->event_pool.push_back(r.e1); }
     m->prof.clear();
     for (int k = 0; k < HUBBARD_N_KCLASS; ++k) { m->prof_launches[k] = 0; m->prof_ms[k] = 0.0; }
     m->profiling = enable != 0;
@@ -1138,8 +1233,8 @@ int hubbard_kernel_times(hubbard_model *m, int64_t *launches, double *ms)
         CU_TRY(m, cudaEventElapsedTime(&t, r.e0, r.e1));
         m->prof_launches[r.kclass] += 1;
         m->prof_ms[r.kclass] += (double)t;
-        cudaEventDestroy(r.e0);
-        cudaEventDestroy(r.e1);
+        m->event_pool.push_back(r.e0);
+        m->event_pool.push_back(r.e1);
     }
     m->prof.clear();
     for (int k = 0; k < HUBBARD_N_KCLASS; ++k) { launches[k] = m->prof_launches[k]; ms[k] = m->prof_ms[k]; }

@@ -288,6 +288,7 @@ gather_sweep_kernel(GatherArgs<T> A)
     const int64_t tile_bytes = (int64_t)n_in_p * (int64_t)sizeof(PR);
     const int n_it = (n_in_w + nthr - 1) / nthr;                // gather iterations per tile
     const int64_t pf_slice = ((tile_bytes + n_it - 1) / n_it + 15) / 16 * 16;       // bytes of the next tile requested per iteration
+    const bool pf_ok = (tile_bytes % 16) == 0;            // bulk prefetches need 16-byte aligned addresses and sizes
     // buffers written in the other sweep's layout
     PR *outW = reinterpret_cast<PR *>(A.Wct);             // ROW: w (or x) in CT
     PR *outZ = reinterpret_cast<PR *>(COL ? A.Frt : A.Zct);   // ROW: z in CT;  COL/LZ: q in RT
@@ -356,7 +357,8 @@ gather_sweep_kernel(GatherArgs<T> A)
             for (int r = 0; r < R; ++r) so[r] = (o0 + r < du) ? A.st_out[o0 + r] : 0u;
         }
         int it = 0;
-        EB pk = load_batch(reinterpret_cast<const EB *>(ent) + threadIdx.x);    // every state has >= 1 (padding) batch
+        // every state has >= 1 (padding) batch; the table has n_in_w batches per plane, a block may have more threads
+        EB pk = load_batch(reinterpret_cast<const EB *>(ent) + min((int)threadIdx.x, n_in_w - 1));
         for (int i = threadIdx.x; i < n_in_w; i += nthr, ++it) {
             const bool valid = i < n_in;
             const bool inpad = i < n_in_p;
@@ -376,7 +378,7 @@ gather_sweep_kernel(GatherArgs<T> A)
 #endif
             // keep DRAM busy during the gather: a slice of the next tile's inputs goes to L2 every iteration
 #if GS_L2PF
-            if ((COL || LZ) && tile + gridDim.x < n_tiles) {
+            if ((COL || LZ) && pf_ok && tile + gridDim.x < n_tiles) {
                 const int64_t off = (int64_t)it * pf_slice + (int64_t)threadIdx.x * 2048;
                 if (threadIdx.x * 2048 < pf_slice && off < tile_bytes) {
                     const unsigned nb = (unsigned)min((int64_t)2048, min(pf_slice - (int64_t)threadIdx.x * 2048, tile_bytes - off));

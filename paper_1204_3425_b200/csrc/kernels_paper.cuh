@@ -23,11 +23,17 @@ struct SweepArgs {
 
 constexpr int kPaperThreads = 256;
 
-template <typename T, bool LANCZOS>
+// SUB = sub-vectors (rows of V) per block = elements per thread.  SUB = 1 is
+// Algorithms 2-4 as printed; SUB = 4 is the paper's own tuning (PAPER.md:338:
+// "four elements per thread, i.e. four subvectors per block"): the block stages
+// the ELL rows of H_up of its SUB sub-vectors ("increases register and shared
+// memory usage") and each down-hop entry Ax/Aj[i * dimDn + id] is loaded once
+// for the SUB elements a thread owns.
+template <typename T, bool LANCZOS, int SUB>
 __global__ void __launch_bounds__(kPaperThreads)
 hv_paper_kernel(DevModel M, SweepArgs<T> A)
 {
-    extern __shared__ uint32_t s_up[];   // w_up entries of the current up row
+    extern __shared__ uint32_t s_up[];   // SUB x w_up entries: the up rows of the block's sub-vectors
     __shared__ double red[32];
     __shared__ int flag;
 
@@ -46,34 +52,48 @@ hv_paper_kernel(DevModel M, SweepArgs<T> A)
     const int ndn = active ? M.dn_cnt[b] : 0;
     const uint32_t sdn = active ? M.st_dn[b] : 0u;
 
-    for (int64_t a = blockIdx.y; a < M.dim_up; a += gridDim.y) {
-        const int nup = M.up_cnt[a];
+    for (int64_t a0 = (int64_t)blockIdx.y * SUB; a0 < M.dim_up; a0 += (int64_t)gridDim.y * SUB) {
+        int nup[SUB];
+#pragma unroll
+        for (int r = 0; r < SUB; ++r) nup[r] = (a0 + r < M.dim_up) ? M.up_cnt[a0 + r] : 0;
         __syncthreads();
-        for (int k = threadIdx.x; k < nup; k += blockDim.x) s_up[k] = M.up_ent[a * M.w_up + k];
+#pragma unroll
+        for (int r = 0; r < SUB; ++r)
+            for (int k = threadIdx.x; k < nup[r]; k += blockDim.x) s_up[r * M.w_up + k] = M.up_ent[(a0 + r) * M.w_up + k];
         __syncthreads();
         if (!active) continue;
-        const T *xa = A.x + a * M.dim_dn;
-        T sum = T(0);
+        T sum[SUB];
         // Algorithm 2: (H_up (x) I) x — whole-row, coalesced reads
-        for (int k = 0; k < nup; ++k) {
-            uint32_t e = s_up[k];
-            sum += signed_by(e, A.x[(int64_t)(e >> 1) * M.dim_dn + b]);
+#pragma unroll
+        for (int r = 0; r < SUB; ++r) {
+            sum[r] = T(0);
+            for (int k = 0; k < nup[r]; ++k) {
+                uint32_t e = s_up[r * M.w_up + k];
+                sum[r] += signed_by(e, A.x[(int64_t)(e >> 1) * M.dim_dn + b]);
+            }
         }
-        // Algorithm 3: (I (x) H_dn) x — gather inside row a
+        // Algorithm 3: (I (x) H_dn) x — gather inside each of the SUB rows, one entry load for all of them
         for (int k = 0; k < ndn; ++k) {
             uint32_t e = M.dn_ent32[(int64_t)k * M.ld_dn + b];
-            sum += signed_by(e, xa[e >> 1]);
+#pragma unroll
+            for (int r = 0; r < SUB; ++r)
+                if (a0 + r < M.dim_up) sum[r] += signed_by(e, A.x[(a0 + r) * M.dim_dn + (e >> 1)]);
         }
-        // Algorithm 4: on-the-fly diagonal
-        const T xv = xa[b];
-        T h = tt * sum + UU * (T)__popc(M.st_up[a] & sdn) * xv;
-        if (LANCZOS) {
-            T *ya = A.y + a * M.dim_dn;
-            T q = c_cur * h - bc * ya[b];
-            ya[b] = q;
-            acc += (double)q * (double)(c_cur * xv);
-        } else {
-            A.y[a * M.dim_dn + b] = h;
+#pragma unroll
+        for (int r = 0; r < SUB; ++r) {
+            const int64_t a = a0 + r;
+            if (a >= M.dim_up) break;
+            // Algorithm 4: on-the-fly diagonal
+            const T xv = A.x[a * M.dim_dn + b];
+            T h = tt * sum[r] + UU * (T)__popc(M.st_up[a] & sdn) * xv;
+            if (LANCZOS) {
+                T *ya = A.y + a * M.dim_dn;
+                T q = c_cur * h - bc * ya[b];
+                ya[b] = q;
+                acc += (double)q * (double)(c_cur * xv);
+            } else {
+                A.y[a * M.dim_dn + b] = h;
+            }
         }
     }
     if (LANCZOS) {

@@ -67,6 +67,24 @@ struct ProfRecord {
     cudaEvent_t e0, e1;
 };
 
+// Development / test knobs, set per model with hubbard_debug_set (include/hubbard.h); the defaults are what
+// bench.py times.  Nothing here is read from the environment.
+struct DebugOptions {
+    int gather_R = 0;               // cap on the tile height R of variant GATHER (0 = none)
+    int gather_nosched = 0;         // 1: hop entries in bond order, no bank-aware placement
+    int gather_ctas = 4;            // CTAs per SM for small tiles
+    int apply_pure_gather = 0;      // 1: plain hubbard_apply as two gather sweeps instead of the hybrid
+    int twosweep_old_row = 0;       // 1: TWOSWEEP fallback keeps the first row kernel
+    int row_R = 0;                  // rows per CTA of the TWOSWEEP row kernel (0 = automatic)
+    int strip_mb = 24;              // L2 budget of a column strip (MB)
+    int strip_rb = 0;               // rows per block of the strip sweep (0 = automatic)
+    int persist_max_dim = 1 << 17;  // largest dim AUTO runs in the cooperative kernel
+    int force_cluster_row = 0;      // 1: take the path of rows larger than one SM
+    int no_cluster_row = 0;         // 1: never use the cluster row sweep
+    int cluster_R = 0, cluster_NC = 0;   // force one (R, NC) of the cluster row sweep
+    int paper_subvectors = 1;       // variant PAPER: sub-vectors per block (1, or 4 = the paper's tuned form)
+};
+
 }  // namespace hub
 
 struct hubbard_model {
@@ -85,6 +103,8 @@ struct hubbard_model {
     int cluster_row = 0;               // rows go through clusters (kernels_cluster.cuh): gather_R == 0 but a cluster holds them
     int cluster_R = 0, cluster_NC = 0, cluster_part = 0;
     int gather_R = 0;                  // tile height of variant GATHER, 0 = does not fit
+    hub::DebugOptions opt;
+    std::vector<void *> layout_allocs;  // device tables that depend on `opt` (rebuilt by hubbard_debug_set)
 
     hub::DevModel dev{};
     std::vector<void *> dev_allocs;    // everything to cudaFree
@@ -103,6 +123,7 @@ struct hubbard_model {
 
     bool profiling = false;
     std::vector<hub::ProfRecord> prof;
+    std::vector<cudaEvent_t> event_pool;   // reused by the profiling scopes
     int64_t prof_launches[HUBBARD_N_KCLASS] = {0};
     double prof_ms[HUBBARD_N_KCLASS] = {0};
 };

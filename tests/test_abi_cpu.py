@@ -226,3 +226,23 @@ def test_expm_e1_vs_scipy():
             y = hb.lanczos_expm_e1(a, b, tau, t)
             ref = expm(-(tau + 1j * t) * T)[:, 0]
             assert np.max(np.abs(y - ref)) <= 1e-11 * max(1.0, np.max(np.abs(ref)))
+
+
+def test_debug_knobs_are_explicit_per_model_state(monkeypatch):
+    """The test / A-B switches are per-model ABI state (hubbard_debug_set), not environment variables: a stray
+    variable cannot reroute a run, unknown keys and out-of-range values are refused."""
+    monkeypatch.setenv("HUBBARD_GATHER_R", "1")          # round-1 name: must have no effect any more
+    c = CONFIGS["C2"]
+    m = hb.hubbard_create_host(c.n_sites, c.n_up, c.n_dn, c.bonds, c.t, 4.0)
+    assert m.hubbard_debug_get("gather_R") == 0
+    m.hubbard_debug_set("gather_R", 2)
+    assert m.hubbard_debug_get("gather_R") == 2
+    m2 = hb.hubbard_create_host(c.n_sites, c.n_up, c.n_dn, c.bonds, c.t, 4.0)
+    assert m2.hubbard_debug_get("gather_R") == 0         # no process-wide state
+    for key, bad in (("gather_R", 5), ("gather_ctas", 0), ("no_such_key", 1), ("cluster_NC", -1)):
+        with pytest.raises(hb.HubbardError):
+            m.hubbard_debug_set(key, bad)
+    with pytest.raises(hb.HubbardError):
+        m.hubbard_debug_get("no_such_key")
+    src = "".join(p.read_text() for p in (ROOT / "paper_1204_3425_b200" / "csrc").glob("*"))
+    assert "getenv" not in src

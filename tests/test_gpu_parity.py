@@ -26,6 +26,22 @@ VARIANTS = {"paper": hb.VARIANT_PAPER, "twosweep": hb.VARIANT_TWOSWEEP, "gather"
             "auto": hb.VARIANT_AUTO}
 
 
+def oracle_record(name, U):
+    """One record of tests/golden/oracle_energies.txt (written by tests/golden/make_energies.py with the oracle
+    only): (iterations, E0, alpha prefix, beta prefix)."""
+    from conftest import read_golden
+    lines = read_golden("oracle_energies.txt")
+    for k, line in enumerate(lines):
+        f = line.split()
+        if f[0] == "case" and f[1] == name and float(f[2]) == float(U):
+            assert int(f[4]) == CONFIGS[name].seed
+            e0 = float(lines[k + 1].split()[1])
+            a = np.array([float(x) for x in lines[k + 2].split()[1:]])
+            b = np.array([float(x) for x in lines[k + 3].split()[1:]])
+            return int(f[3]), e0, a, b
+    raise KeyError((name, U))
+
+
 def dev():
     assert torch.cuda.is_available(), "these tests need the B200 (no CPU fallback exists)"
     return torch.device("cuda:0")
@@ -85,14 +101,15 @@ def test_apply_vs_definition_small(ns, nu, nd, bonds, dtype, variant):
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 @pytest.mark.parametrize("R", [1, 2])
-def test_gather_narrow_tiles(R, dtype, monkeypatch):
+def test_gather_narrow_tiles(R, dtype):
     """Variant GATHER with tile heights below the 16-byte width (what a large
     sector would get: C5 fp32 has R = 1): H*v on C2 and a short Lanczos run,
-    forced through HUBBARD_GATHER_R (read by hubbard_create)."""
-    monkeypatch.setenv("HUBBARD_GATHER_R", str(R))
+    forced through hubbard_debug_set("gather_R")."""
     c = CONFIGS["C2"]
     ref = RefModel(c.n_sites, c.n_up, c.n_dn, c.bonds, c.t, 4.0)
     m = hb.hubbard_create(c.n_sites, c.n_up, c.n_dn, c.bonds, c.t, 4.0, dtype)
+    m.hubbard_debug_set("gather_R", R)
+    assert m.hubbard_debug_get("resolved_gather_R") == R
     m.hubbard_set_variant(hb.VARIANT_GATHER)
     x, x_np = start_vector(c.seed, c.dim, dtype)
     y = torch.full_like(x, float("nan"))
@@ -140,6 +157,44 @@ def test_apply_full_vector_C4(dtype):
     m.hubbard_apply(x, y)
     torch.cuda.synchronize()
     assert rel_max_err(y, y_ref) <= TOL_HV[dtype]
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_paper_comparator_four_subvectors_per_block(dtype):
+    """SURVEY 8(f)-1, second half: the paper's tuned comparator (four sub-vectors per block = four
+    elements per thread) - H*v on small ragged sectors (dim_up not a multiple of 4, dim_up < 4) against the dense
+    definitional H, on C2 against the tier-1 oracle, and a Lanczos run."""
+    for ns, nu, nd, bonds in SMALL:
+        H = hd.dense_hamiltonian(ns, nu, nd, bonds, 0.75, 3.5)
+        m = hb.hubbard_create(ns, nu, nd, bonds, 0.75, 3.5, dtype)
+        m.hubbard_set_variant(hb.VARIANT_PAPER)
+        m.hubbard_debug_set("paper_subvectors", 4)
+        x, x_np = start_vector(77 + ns, m.dim, dtype)
+        y = torch.full_like(x, float("nan"))
+        m.hubbard_apply(x, y)
+        torch.cuda.synchronize()
+        y_ref = H @ x_np
+        if np.max(np.abs(y_ref)) == 0.0:
+            assert float(y.abs().max()) == 0.0
+        else:
+            assert rel_max_err(y, y_ref) <= TOL_HV[dtype]
+    c = CONFIGS["C2"]
+    ref = RefModel(c.n_sites, c.n_up, c.n_dn, c.bonds, c.t, 4.0)
+    m = hb.hubbard_create(c.n_sites, c.n_up, c.n_dn, c.bonds, c.t, 4.0, dtype)
+    m.hubbard_set_variant(hb.VARIANT_PAPER)
+    m.hubbard_debug_set("paper_subvectors", 4)
+    x, x_np = start_vector(c.seed, c.dim, dtype)
+    y = torch.full_like(x, float("nan"))
+    m.hubbard_apply(x, y)
+    torch.cuda.synchronize()
+    assert rel_max_err(y, ref.apply(x_np)) <= TOL_HV[dtype]
+    alpha, beta = m.lanczos_run(x, 60)
+    a_ref, b_ref = lr.lanczos(ref.apply, x_np, 60)
+    n = 30
+    tol_c = 1e-10 if dtype == "f64" else 1e-5
+    assert np.max(np.abs(alpha[:n] - a_ref[:n]) / np.maximum(1.0, np.abs(a_ref[:n]))) <= tol_c
+    e_ref = lr.ground_energy(a_ref, b_ref)
+    assert abs(hb.lanczos_ground_energy(alpha, beta) - e_ref) <= TOL_E0[dtype] * abs(e_ref)
 
 
 def _sampled_parity(name, dtype, n_samples, U):
@@ -272,6 +327,119 @@ def test_lanczos_C3_prefix(dtype, n_prefix):
     _lanczos_case("C3", 8.0, dtype, "auto", 40, n_prefix)
 
 
+def _lanczos_vs_golden(name, U, dtype, n_prefix):
+    """Full-length run in the launch configuration bench.py times (variant AUTO) against the stored oracle run
+    (Algorithm 1 verbatim on the tier-1 H*v, same seeded start vector): E_0 after the configuration's fixed
+    iteration count (north_star: <= 1e-10 / 1e-5 relative) and the coefficient prefix of reading Q12."""
+    c = CONFIGS[name]
+    iters, e_ref, a_ref, b_ref = oracle_record(name, U)
+    assert iters == c.iters
+    m = hb.hubbard_create(c.n_sites, c.n_up, c.n_dn, c.bonds, c.t, U, dtype)
+    v0, _ = start_vector(c.seed, c.dim, dtype)
+    alpha, beta = m.lanczos_run(v0, iters)
+    assert len(alpha) == iters
+    tol_c = 1e-10 if dtype == "f64" else 1e-5
+    n = min(n_prefix, len(a_ref))
+    assert np.max(np.abs(alpha[:n] - a_ref[:n]) / np.maximum(1.0, np.abs(a_ref[:n]))) <= tol_c
+    assert np.max(np.abs(beta[:n] - b_ref[:n]) / np.maximum(1.0, np.abs(b_ref[:n]))) <= tol_c
+    e_gpu = hb.lanczos_ground_energy(alpha, beta)
+    assert abs(e_gpu - e_ref) <= TOL_E0[dtype] * abs(e_ref)
+    return e_gpu
+
+
+@pytest.mark.parametrize("dtype,n_prefix", [("f64", 50), ("f32", 30)])
+def test_lanczos_C3_full_vs_oracle(dtype, n_prefix):
+    """C3 at its full 200 iterations."""
+    e = _lanczos_vs_golden("C3", 8.0, dtype, n_prefix)
+    assert abs(e - (-17.510366694879)) < 1e-4            # SURVEY P11 (sanity only)
+
+
+@pytest.mark.parametrize("dtype,n_prefix", [("f64", 50), ("f32", 30)])
+@pytest.mark.parametrize("U", [4.0, 8.0])
+def test_lanczos_C4_full_vs_oracle(U, dtype, n_prefix):
+    """The headline configuration: E_0 after the fixed 200 iterations, U = 4 and U = 8, both dtypes."""
+    _lanczos_vs_golden("C4", U, dtype, n_prefix)
+
+
+def _c5_fits(dtype, n_vec):
+    free, _ = torch.cuda.mem_get_info()
+    need = n_vec * CONFIGS["C5"].dim * (8 if dtype == "f64" else 4) + (4 << 30)
+    if free < need:
+        pytest.skip(f"needs {need >> 30} GiB of free HBM")
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_lanczos_C5_first_iterations_vs_oracle(dtype):
+    """C5 (dim = 2 363 904 400 > 2^31) through lanczos_run under AUTO - the cluster (DSMEM) row sweep in its
+    Lanczos form for fp64, the row-major gather ROW sweep for fp32, the <LZ> strip sweep and the axpy+norm kernel
+    with 64-bit offsets: a_1, b_2, a_2, b_3 against Algorithm 1 written out on the tier-1 oracle over the FULL
+    vector (tests/golden/make_energies.py C5: two resident host vectors of 18.9 GB)."""
+    _c5_fits(dtype, 3)
+    c = CONFIGS["C5"]
+    iters, _, a_ref, b_ref = oracle_record("C5", 4.0)
+    m = hb.hubbard_create(c.n_sites, c.n_up, c.n_dn, c.bonds, c.t, 4.0, dtype)
+    assert m.hubbard_debug_get("resolved_variant") == hb.VARIANT_TWOSWEEP
+    v0 = start_vector_torch(c.seed, c.dim, dev(), TDT[dtype])     # un-normalised: lanczos_run normalises its copy
+    alpha, beta = m.lanczos_run(v0, iters)
+    del v0
+    tol = 1e-10 if dtype == "f64" else 1e-5
+    assert len(alpha) == iters == 2
+    assert np.max(np.abs(alpha - a_ref) / np.maximum(1.0, np.abs(a_ref))) <= tol
+    assert np.max(np.abs(beta - b_ref) / np.maximum(1.0, np.abs(b_ref))) <= tol
+    m.close()
+    torch.cuda.empty_cache()
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_lanczos_C5_free_fermions(dtype):
+    """Pin P6 at full scale, oracle-free: U = 0 on the half-filled 18-ring, E_0 = 2 * sum of the 9 lowest levels
+    of -2 cos(2 pi n / 18) = -23.035081932575 (closed shell).  Any wrong wrap sign, 32-bit offset or DSMEM
+    index would move it."""
+    _c5_fits(dtype, 3)
+    c = CONFIGS["C5"]
+    e_exact = 2.0 * sum(sorted(-2.0 * np.cos(2.0 * np.pi * np.arange(18) / 18.0))[:9])
+    assert abs(e_exact - (-23.035081932575)) < 1e-11
+    m = hb.hubbard_create(c.n_sites, c.n_up, c.n_dn, c.bonds, c.t, 0.0, dtype)
+    v0 = start_vector_torch(c.seed, c.dim, dev(), TDT[dtype])
+    alpha, beta, e0 = m.lanczos_run_until(v0, 300, check_every=20, tol=1e-13 if dtype == "f64" else 1e-7)
+    del v0
+    assert abs(e0 - e_exact) <= TOL_E0[dtype] * abs(e_exact), (len(alpha), e0)
+    m.close()
+    torch.cuda.empty_cache()
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("name,ns,nu,nd,bonds", [("C2", 12, 6, 6, ring_bonds(12)), ("odd", 13, 5, 7, ring_bonds(13) + [(0, 5)])])
+def test_auto_twosweep_with_gather_row(name, ns, nu, nd, bonds, dtype):
+    """The path C5 fp32 takes under AUTO, on sectors the oracle covers in full: the gather tile is narrower than
+    16 bytes (forced with gather_R = 1), so AUTO resolves to TWOSWEEP whose row half is the gather ROW sweep in
+    its ROW-MAJOR Lanczos form (eq. 13 folded: y = c (t H_dn + D) x - b_j c_{j-1} y), followed by the <LZ> strip
+    sweep and the axpy+norm kernel."""
+    ref = RefModel(ns, nu, nd, bonds, 1.0, 4.0)
+    m = hb.hubbard_create(ns, nu, nd, bonds, 1.0, 4.0, dtype)
+    m.hubbard_debug_set("gather_R", 1)
+    m.hubbard_debug_set("persist_max_dim", 0)
+    assert m.hubbard_debug_get("resolved_gather_R") == 1
+    assert m.hubbard_debug_get("resolved_variant") == hb.VARIANT_TWOSWEEP
+    x, x_np = start_vector(77, m.dim, dtype)
+    y = torch.full_like(x, float("nan"))
+    m.hubbard_apply(x, y)
+    torch.cuda.synchronize()
+    assert rel_max_err(y, ref.apply(x_np)) <= TOL_HV[dtype]
+    m.hubbard_profile(True)
+    alpha, beta = m.lanczos_run(x, 40)
+    kt = m.hubbard_kernel_times()
+    m.hubbard_profile(False)
+    assert kt["row_sweep"][0] == 40 and kt["col_sweep"][0] == 40 and kt["vec_sweep"][0] == 40
+    a_ref, b_ref = lr.lanczos(ref.apply, x_np, 40)
+    tol_c = 1e-10 if dtype == "f64" else 1e-5
+    n = 30
+    assert np.max(np.abs(alpha[:n] - a_ref[:n]) / np.maximum(1.0, np.abs(a_ref[:n]))) <= tol_c
+    assert np.max(np.abs(beta[:n] - b_ref[:n]) / np.maximum(1.0, np.abs(b_ref[:n]))) <= tol_c
+    e_ref = lr.ground_energy(a_ref, b_ref)
+    assert abs(hb.lanczos_ground_energy(alpha, beta) - e_ref) <= TOL_E0[dtype] * abs(e_ref)
+
+
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 def test_lanczos_C4_free_fermions(dtype):
     """Pin P6 at full scale, oracle-free: U = 0 on the 4x4 half-filled torus,
@@ -370,14 +538,16 @@ def test_ground_state_vector_small(dtype, variant):
     m.hubbard_set_variant(VARIANTS[variant])
     v0, _ = start_vector(11, m.dim, dtype)
     psi = torch.empty_like(v0)
-    e0, done = m.lanczos_ground_state(v0, 80, psi)
+    # 60 iterations: E_0 has converged, and the accumulated vector is not yet degraded by the loss of
+    # orthogonality that follows convergence (the ORACLE's own residual goes 3e-15 at m = 60 -> 1.3e-11 at m = 80,
+    # DESIGN.md section 5), so the bound below is a statement about the kernels, not about Lanczos
+    e0, done = m.lanczos_ground_state(v0, 60, psi)
     tol = 1e-9 if dtype == "f64" else 2e-4
     assert abs(e0 - w[0]) <= (1e-10 if dtype == "f64" else 1e-5) * abs(w[0])
     p = psi.double().cpu().numpy()
     assert abs(np.linalg.norm(p) - 1.0) < (1e-12 if dtype == "f64" else 1e-6)
     assert abs(abs(np.dot(p, v[:, 0])) - 1.0) <= tol
-    # overlap deficit d bounds the vector error by sqrt(2 d) ~ 4e-5, the residual by that times |H|
-    assert np.max(np.abs(H @ p - e0 * p)) <= (1e-5 if dtype == "f64" else 1e-3)
+    assert np.max(np.abs(H @ p - e0 * p)) <= (1e-7 if dtype == "f64" else 1e-3)
     st_up, st_dn = m.hubbard_get_basis(0), m.hubbard_get_basis(1)
     # an observable is linear in the vector error (the overlap is quadratic in it)
     assert abs(_double_occupancy(p, st_up, st_dn) - _double_occupancy(v[:, 0], st_up, st_dn)) <= (1e-6 if dtype == "f64" else 2e-3)
@@ -503,15 +673,18 @@ def test_propagate_C2_properties():
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 @pytest.mark.parametrize("R,NC", [(0, 0), (1, 2), (1, 4), (2, 2), (2, 4)])
 @pytest.mark.parametrize("name,ns,nu,nd,bonds", [("C2", 12, 6, 6, ring_bonds(12)), ("odd", 13, 5, 7, ring_bonds(13) + [(0, 5)])])
-def test_cluster_row_sweep(name, ns, nu, nd, bonds, R, NC, dtype, monkeypatch):
+def test_cluster_row_sweep(name, ns, nu, nd, bonds, R, NC, dtype):
     """The distributed-shared-memory row sweep (clusters of NC CTAs holding R rows, kernels_cluster.cuh: what
     C5 fp64 uses because a V row exceeds one SM) forced on sectors the oracle covers in full: H*v and a Lanczos
     run; dim_dn not a multiple of 32 or of the cluster split, N_up != N_dn, odd dim_up with R = 2."""
-    monkeypatch.setenv("HUBBARD_FORCE_CLUSTER_ROW", "1")
-    monkeypatch.setenv("HUBBARD_CLUSTER_R", str(R))
-    monkeypatch.setenv("HUBBARD_CLUSTER_NC", str(NC))
     ref = RefModel(ns, nu, nd, bonds, 1.0, 4.0)
     m = hb.hubbard_create(ns, nu, nd, bonds, 1.0, 4.0, dtype)
+    m.hubbard_debug_set("force_cluster_row", 1)
+    m.hubbard_debug_set("cluster_R", R)
+    m.hubbard_debug_set("cluster_NC", NC)
+    assert m.hubbard_debug_get("resolved_cluster_row") == 1 and m.hubbard_debug_get("resolved_gather_R") == 0
+    if R:
+        assert (m.hubbard_debug_get("resolved_cluster_R"), m.hubbard_debug_get("resolved_cluster_NC")) == (R, NC)
     x, x_np = start_vector(77, m.dim, dtype)
     y = torch.full_like(x, float("nan"))
     m.hubbard_apply(x, y)

@@ -356,3 +356,35 @@ def test_P9_spin_swap_tier1():
     y1 = ref.apply(V.T.copy().ravel()).reshape(ref.dim_up, ref.dim_dn)
     y2 = ref.apply(V.ravel()).reshape(ref.dim_up, ref.dim_dn).T
     assert np.abs(y1 - y2).max() < 1e-13
+
+
+def test_fig1_ell_worked_example_pins_hop_ell(golden):
+    """PAPER.md:208-226 (Fig. 1): the 4x4 example matrix, its ELL `data` / `indices` arrays (width = max nnz per
+    row, zero padding printed as *) and their column-major flattening.  Pins RefModel.hop_ell - the CSR -> ELL
+    reformatting whose output is the expected value of the library's hubbard_get_hops in tests/test_abi_cpu.py -
+    against values the paper prints: a dropped entry, a wrong width, row/column-major confusion or a shifted
+    padding would each change the flattened arrays."""
+    lines = golden("paper_ell_example.txt")
+    k = lines.index("A")
+    A = np.array([[float(x) for x in lines[k + 1 + r].split()] for r in range(4)])
+    data = lines[lines.index("data_colmajor") + 1].split()
+    idx = lines[lines.index("indices_colmajor") + 1].split()
+    # the example matrix in CSR, rows in order, columns ascending (as Fig. 1 lists them)
+    rp, cj, cv = [0], [], []
+    for r in range(4):
+        for c in range(4):
+            if A[r, c] != 0.0:
+                cj.append(c)
+                cv.append(A[r, c])
+        rp.append(len(cj))
+    m = RefModel.__new__(RefModel)                       # hop_ell needs only .csr
+    m.csr = {0: (np.array(rp, dtype=np.int64), np.array(cj, dtype=np.int32), np.array(cv, dtype=np.float64))}
+    width, cols, vals = m.hop_ell(0)
+    assert width == 3 == len(data) // 4                  # "the maximum number of nonzeros per row", PAPER.md:228
+    got_data = vals.T.reshape(-1)                        # column-major flattening, PAPER.md:226,230
+    got_idx = cols.T.reshape(-1)
+    for g_d, g_i, w_d, w_i in zip(got_data, got_idx, data, idx):
+        if w_d == "*":
+            assert g_d == 0.0 and g_i == -1              # padding: the paper zero-fills, the canonical form marks col = -1
+        else:
+            assert g_d == float(w_d) and g_i == int(w_i)
