@@ -70,6 +70,8 @@ def parse_args():
     p.add_argument("--iters", type=int, default=None, help="Lanczos iterations per step (default: the config's)")
     p.add_argument("--variant", default="auto", choices=["auto", "paper", "twosweep", "gather", "persist"])
     p.add_argument("--no-extras", action="store_true", help="skip the context rows (plain apply, NEXT rows, comparator)")
+    p.add_argument("--debug", action="append", default=[], metavar="KEY=VALUE",
+                   help="hubbard_debug_set(KEY, VALUE) on the model (A/B measurements; recorded in config)")
     p.add_argument("--no-cpu-baseline", action="store_true")
     p.add_argument("--no-e2e", action="store_true")
     return p.parse_args()
@@ -275,6 +277,9 @@ def run_native_dtype(args, cfg, U, dtype, rank, world, local):
                "gather": hb.VARIANT_GATHER, "persist": hb.VARIANT_PERSIST}[args.variant]
 
     m = hb.hubbard_create(cfg.n_sites, cfg.n_up, cfg.n_dn, cfg.bonds, cfg.t, U, dtype)
+    for kv in args.debug:
+        k, v = kv.split("=")
+        m.hubbard_debug_set(k, int(v))
     m.hubbard_set_variant(variant)
     v0 = start_vector_torch(cfg.seed + rank, cfg.dim, dev, torch.float64)
     v0 /= torch.linalg.vector_norm(v0)
@@ -477,7 +482,8 @@ def main():
                        "start_vector": f"seeded uniform[-1,1) normalised, seed {cfg.seed}+rank",
                        "l2": "inputs exceed L2 (no flush needed)" if cfg.dim * 4 > 2 * 126e6 else
                              "inputs fit in L2: cache-resident by design (DESIGN.md), HBM fraction not meaningful",
-                       "variant": args.variant, "parallelism": "replicas" if world > 1 else "single GPU"},
+                       "variant": args.variant, "debug": args.debug,
+                       "parallelism": "replicas" if world > 1 else "single GPU"},
             "s_per_iteration": main_r["s_per_iteration"],
             "roofline": main_r["roofline"], "kernels": main_r["kernels"], "e2e": main_r["e2e"],
             "gpu_launches": main_r["gpu_launches"], "clocks": main_r["clocks"], "E0": main_r["E0"],

@@ -206,18 +206,33 @@ int hubbard_get_hops(const hubbard_model *m, int spin, int *width,
 
 /* hubbard_get_gather_table: the DEVICE layout of one spin's hop table as variant
  * GATHER uses it (host computation only; works on hubbard_create_host models):
- * the ELL format of PAPER.md:208-230 with batches of 8 entries of one state
- * contiguous - entry k of state i at [((k / 8) * ld + i) * 8 + k % 8], entry =
- * col * 2 + neg (element = t * (neg ? -1 : +1)) - and a state's
- * entries placed in its slots so that the `lanes` lanes served by one
- * shared-memory wavefront (8, 16 or 32; 0 = keep bond order) hit distinct banks.
- * Padding entries have col >= zero_base (>= dim_spin: the zero slots of the
- * staged tile).  Call first with entries_host == counts_host == NULL to obtain
- * *slots (entries per state, a multiple of 8) and *ld; then pass
- * entries_host[*ld * *slots] and counts_host[dim_spin] (last used slot + 1).
- * *conflicts = entries that share a bank with another lane of their wavefront. */
-int hubbard_get_gather_table(const hubbard_model *m, int spin, int lanes, int64_t zero_base, int *slots, int64_t *ld,
-                             uint32_t *entries_host, int32_t *counts_host, int64_t *conflicts);
+ * the ELL format of PAPER.md:208-230 over an INTERNAL order of the spin's basis
+ * states (position p holds state perm[p] of the ascending list of PAPER.md:63-67;
+ * sorted == 2: orbits of a group of `lanes` lattice symmetries as aligned groups,
+ * ordered by descending hop count - equal row lengths inside a group and no bank
+ * conflicts by construction, see csrc/gather_tables.h - falling back to sorted ==
+ * 1 when the bond list has no such group; sorted == 1: aligned groups of `lanes`
+ * consecutive states ordered by descending hop count; sorted == 0: perm =
+ * identity, what the row-major vectors of hubbard_apply need), with
+ * batches of 8 entries of one position contiguous - entry k of position p at
+ * [((k / 8) * ld + p) * 8 + k % 8], entry = target_position * 2 + neg (element =
+ * t * (neg ? -1 : +1)) - and a position's entries placed in its
+ * slots so that the `lanes` lanes served by one shared-memory wavefront (8, 16 or
+ * 32; 0 = keep bond order) hit distinct banks.  R (1, 2 or 4) is the tile height:
+ * the tile holds n_pos = dim_spin rounded up to R positions followed by `lanes`
+ * zero slots, and padding entries have target_position >= n_pos.
+ * Call first with the array arguments NULL to obtain *slots (entries per position
+ * in the table, a multiple of 8) and *ld (a multiple of 32, >= n_pos); then pass
+ *   entries_host[*ld * *slots], counts_host[*ld] (last slot holding a real entry + 1),
+ *   warp_slots_host[*ld / 32] (the EXACT number of slots every lane of that warp of
+ *   32 positions walks; slots below it hold real or zero-slot entries),
+ *   perm_host[*ld] (position -> state index, -1 for padding positions).
+ * *conflicts = entries that share a bank with another lane of their wavefront;
+ * *wavefronts = shared-memory wavefronts one tile's gather costs in this layout
+ * (sum over warps of warp_slots * 32 / lanes, plus the conflicts' replays). */
+int hubbard_get_gather_table(const hubbard_model *m, int spin, int lanes, int R, int sorted, int *slots, int64_t *ld,
+                             uint32_t *entries_host, int32_t *counts_host, uint16_t *warp_slots_host, int32_t *perm_host,
+                             int64_t *conflicts, int64_t *wavefronts);
 
 /* ---- host utility, off the hot path ----
  * e0 = smallest eigenvalue of the symmetric tridiagonal T_m with diagonal
@@ -248,6 +263,8 @@ int64_t hubbard_launch_count(const hubbard_model *m);
  * states what it forces; the defaults are what bench.py times and what production callers get.  Keys (value range):
  *   "gather_R" (0-4)          cap on the tile height R of variant GATHER, 0 = none (what a larger sector would get)
  *   "gather_nosched" (0/1)    hop entries in bond order, no bank-aware placement
+ *   "gather_nosort" (0/1)     the Lanczos work vectors of variant GATHER keep the basis order
+ *   "gather_nosymmetry" (0/1) their internal order comes from hop counts only (no lattice-symmetry orbits)
  *   "gather_ctas" (1-4)       CTAs per SM for small tiles
  *   "apply_pure_gather" (0/1) plain hubbard_apply as two gather sweeps instead of the hybrid
  *   "twosweep_old_row" (0/1)  AUTO's TWOSWEEP fallback keeps the first row kernel
@@ -259,7 +276,8 @@ int64_t hubbard_launch_count(const hubbard_model *m);
  *                             take / avoid the cluster row sweep of rows larger than one SM, force one (R, NC)
  * Options that change a device table layout re-upload that table (host work + cudaMemcpy; no kernel launch).
  * hubbard_debug_get returns an option, or what the library resolved for this model: "resolved_variant"
- * (HUBBARD_VARIANT_* that AUTO stands for), "resolved_gather_R", "resolved_cluster_row", "resolved_cluster_R",
+ * (HUBBARD_VARIANT_* that AUTO stands for), "resolved_gather_R", "resolved_gather_symmetry" (order of the lattice symmetry group the
+ * internal order of variant GATHER was built from, 0 = none), "resolved_cluster_row", "resolved_cluster_R",
  * "resolved_cluster_NC".  Unknown key or out-of-range value: HUBBARD_ERR_INVALID. */
 int hubbard_debug_set(hubbard_model *m, const char *key, int value);
 int hubbard_debug_get(const hubbard_model *m, const char *key, int *value);

@@ -56,7 +56,8 @@ def _load() -> C.CDLL:
     lib.lanczos_run_host.argtypes = [vp, vp, i32, P(dbl), P(dbl), P(i32), vp]
     lib.hubbard_get_basis.argtypes = [vp, i32, P(C.c_uint32)]
     lib.hubbard_get_hops.argtypes = [vp, i32, P(i32), P(C.c_int32), P(dbl)]
-    lib.hubbard_get_gather_table.argtypes = [vp, i32, i32, i64, P(i32), P(i64), P(C.c_uint32), P(C.c_int32), P(i64)]
+    lib.hubbard_get_gather_table.argtypes = [vp, i32, i32, i32, i32, P(i32), P(i64), P(C.c_uint32), P(C.c_int32),
+                                             P(C.c_uint16), P(C.c_int32), P(i64), P(i64)]
     lib.lanczos_ground_energy.argtypes = [P(dbl), P(dbl), i32, P(dbl)]
     lib.hubbard_profile.argtypes = [vp, i32]
     lib.hubbard_kernel_times.argtypes = [vp, P(i64), P(dbl)]
@@ -244,19 +245,24 @@ class Model:
                                     vals.ctypes.data_as(C.POINTER(C.c_double))), "hubbard_get_hops")
         return w.value, cols, vals
 
-    def hubbard_get_gather_table(self, spin, lanes, zero_base=None):
-        """(slots, ld, entries[slots/8, ld, 8], counts[dim_spin], conflicts) of variant GATHER's table."""
-        n = self.dim_up if spin == 0 else self.dim_dn
-        zb = n if zero_base is None else int(zero_base)
-        w, ld, cf = C.c_int(0), C.c_int64(0), C.c_int64(0)
-        _check(lib.hubbard_get_gather_table(self._h, spin, lanes, zb, C.byref(w), C.byref(ld), None, None, C.byref(cf)),
-               "hubbard_get_gather_table")
+    def hubbard_get_gather_table(self, spin, lanes, R=1, sorted=False):
+        """Variant GATHER's table: dict(slots, ld, entries[slots/8, ld, 8], counts[ld], warp_slots[ld/32], perm[ld],
+        conflicts, wavefronts)."""
+        w, ld, cf, wf = C.c_int(0), C.c_int64(0), C.c_int64(0), C.c_int64(0)
+        _check(lib.hubbard_get_gather_table(self._h, spin, lanes, R, int(sorted), C.byref(w), C.byref(ld), None, None,
+                                            None, None, C.byref(cf), C.byref(wf)), "hubbard_get_gather_table")
         ent = np.empty((w.value // 8, ld.value, 8), dtype=np.uint32)
-        cnt = np.empty(n, dtype=np.int32)
-        _check(lib.hubbard_get_gather_table(self._h, spin, lanes, zb, C.byref(w), C.byref(ld),
+        cnt = np.empty(ld.value, dtype=np.int32)
+        wsl = np.empty(ld.value // 32, dtype=np.uint16)
+        perm = np.empty(ld.value, dtype=np.int32)
+        _check(lib.hubbard_get_gather_table(self._h, spin, lanes, R, int(sorted), C.byref(w), C.byref(ld),
                                             ent.ctypes.data_as(C.POINTER(C.c_uint32)),
-                                            cnt.ctypes.data_as(C.POINTER(C.c_int32)), C.byref(cf)), "hubbard_get_gather_table")
-        return w.value, ld.value, ent, cnt, cf.value
+                                            cnt.ctypes.data_as(C.POINTER(C.c_int32)),
+                                            wsl.ctypes.data_as(C.POINTER(C.c_uint16)),
+                                            perm.ctypes.data_as(C.POINTER(C.c_int32)), C.byref(cf), C.byref(wf)),
+               "hubbard_get_gather_table")
+        return {"slots": w.value, "ld": ld.value, "entries": ent, "counts": cnt, "warp_slots": wsl, "perm": perm,
+                "conflicts": cf.value, "wavefronts": wf.value}
 
     # -- measurement hooks
     def hubbard_profile(self, enable=True):

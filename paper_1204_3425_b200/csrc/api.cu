@@ -116,22 +116,26 @@ bool cluster_row_config(const hubbard_model *m, int *R_out, int *NC_out, int *pa
 }
 
 // Hop table of one spin for variant GATHER (kernels_gather.cuh, gather_tables.h).
-int upload_gather_table(hubbard_model *m, const SpinTable &tab, const uint32_t *d_states, int R, SpinDev *out)
+int upload_gather_table(hubbard_model *m, const SpinTable &tab, int R, bool sorted, SpinDev *out)
 {
     SpinDev G{};
-    G.dim = tab.dim;
-    G.st = d_states;
     const int es = m->dtype == HUBBARD_F32 ? 4 : 8;
     const int lanes = m->opt.gather_nosched ? 0 : 128 / (R * es);
     GatherTable T;
-    build_gather_table(tab, lanes, (tab.dim + R - 1) / R * R, T);
-    G.w = T.w;
-    G.ld = T.ld;
+    const bool sym = sorted && !m->opt.gather_nosymmetry;
+    build_gather_table(tab, lanes, R, sorted && !m->opt.gather_nosort, T, sym ? m->bonds.data() : nullptr,
+                       sym ? (int)(m->bonds.size() / 2) : 0);
+    if (sorted) m->gather_symmetry = T.symmetry_order;
+    G.dim = tab.dim; G.n_pos = T.n_pos; G.ld = T.ld; G.w = T.w;
     int rc;
     if ((rc = dev_upload(m, T.ent, &G.e32, true))) return rc;
-    if ((rc = dev_upload(m, T.cnt, &G.cnt, true))) return rc;
+    if ((rc = dev_upload(m, T.wslots, &G.wslots, true))) return rc;
+    if ((rc = dev_upload(m, T.perm, &G.perm, true))) return rc;
+    std::vector<uint32_t> st((size_t)T.ld, 0u);
+    for (int64_t p = 0; p < tab.dim; ++p) st[(size_t)p] = tab.states[(size_t)T.perm[(size_t)p]];
+    if ((rc = dev_upload(m, st, &G.st, true))) return rc;
     G.e16 = nullptr;
-    if (tab.dim + 1 + 128 <= 32768) {
+    if (T.n_pos + 128 <= 32768) {
         std::vector<uint16_t> e16(T.ent.size());
         for (size_t i = 0; i < T.ent.size(); ++i) e16[i] = (uint16_t)T.ent[i];
         if ((rc = dev_upload(m, e16, &G.e16, true))) return rc;
@@ -147,18 +151,20 @@ int upload_layout_tables(hubbard_model *m)
     DevModel &D = m->dev;
     for (void *p : m->layout_allocs) cudaFree(p);
     m->layout_allocs.clear();
-    D.g_up = SpinDev{}; D.g_dn = SpinDev{};
+    D.g_up = SpinDev{}; D.g_dn = SpinDev{}; D.gs_up = SpinDev{}; D.gs_dn = SpinDev{};
     m->cluster_row = 0; m->cluster_R = m->cluster_NC = m->cluster_part = 0;
     int rc;
     try {
         // variant GATHER: both spins column-major, entry = col * 2 + neg
         m->gather_R = gather_R_for(m);
         if (m->gather_R > 0) {
-            if ((rc = upload_gather_table(m, m->up, D.st_up, m->gather_R, &D.g_up))) return rc;
-            if ((rc = upload_gather_table(m, m->dn, D.st_dn, m->gather_R, &D.g_dn))) return rc;
+            if ((rc = upload_gather_table(m, m->up, m->gather_R, false, &D.g_up))) return rc;
+            if ((rc = upload_gather_table(m, m->dn, m->gather_R, false, &D.g_dn))) return rc;
+            if ((rc = upload_gather_table(m, m->up, m->gather_R, true, &D.gs_up))) return rc;
+            if ((rc = upload_gather_table(m, m->dn, m->gather_R, true, &D.gs_dn))) return rc;
         } else if (cluster_row_config(m, &m->cluster_R, &m->cluster_NC, &m->cluster_part)) {
             // R rows fit the shared memory of a cluster: down-spin table in that layout for kernels_cluster.cuh
-            if ((rc = upload_gather_table(m, m->dn, D.st_dn, m->cluster_R, &D.g_dn))) return rc;
+            if ((rc = upload_gather_table(m, m->dn, m->cluster_R, false, &D.g_dn))) return rc;
             m->cluster_row = 1;
         }
     } catch (const std::bad_alloc &) {
@@ -323,10 +329,8 @@ int launch_gather_inst(hubbard_model *m, GatherArgs<T> A, cudaStream_t st)
     A.du_p = round_up(A.dim_up, R);
     A.dd_p = round_up(A.dim_dn, R);
     const int64_t n_in_p = COL ? A.du_p : A.dd_p;
-    size_t smem = (size_t)(n_in_p + 128 / (R * sizeof(T))) * R * sizeof(T);
-    const size_t cnt_bytes = (size_t)round_up(n_in_p, 32);
-    A.cnt_in_smem = (A.in.w < 256 && smem + cnt_bytes + 1024 <= (size_t)m->max_smem_optin) ? 1 : 0;
-    if (A.cnt_in_smem) smem += cnt_bytes;
+    // the staged tile + its zero slots, then the per-warp slot counts
+    const size_t smem = (size_t)(n_in_p + 128 / (R * sizeof(T))) * R * sizeof(T) + (size_t)(round_up(n_in_p, 32) / 32) * sizeof(uint16_t);
     if (int rc = ensure_smem(m, kern, smem, true)) return rc;
     const int64_t tiles = (COL ? A.dd_p : A.du_p) / R;
     // Small sectors: several CTAs per SM (their staging and gather phases overlap one another); the 64-register
@@ -342,12 +346,13 @@ int launch_gather_inst(hubbard_model *m, GatherArgs<T> A, cudaStream_t st)
     return after_launch(m);
 }
 
+// LZ: the Lanczos sweeps work in the sorted internal order of BOTH spins; plain apply (row-major callers) in basis order.
 template <typename T, bool COL, bool LZ>
 int launch_gather(hubbard_model *m, GatherArgs<T> A, cudaStream_t st)
 {
     const DevModel &D = m->dev;
-    A.in = COL ? D.g_up : D.g_dn;
-    A.st_out = D.st_up;
+    A.in = LZ ? (COL ? D.gs_up : D.gs_dn) : (COL ? D.g_up : D.g_dn);
+    A.st_out = LZ ? D.gs_up.st : D.st_up;
     A.dim_up = D.dim_up; A.dim_dn = D.dim_dn; A.t = m->t; A.U = m->U;
     const int R = gather_R(m);
     if (R == 0) return HUBBARD_ERR_INVALID;
@@ -371,11 +376,12 @@ int launch_to_rt(hubbard_model *m, const T *x, T *rt, cudaStream_t st)
     const int R = gather_R(m);
     const int64_t du = m->up.dim, dd = m->dn.dim, du_p = round_up(du, R), dd_p = round_up(dd, R);
     const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((int64_t)m->sm_count * 8, (du_p / R * dd_p + 255) / 256));
+    const int32_t *pu = m->dev.gs_up.perm, *pd = m->dev.gs_dn.perm;
     if constexpr (sizeof(T) == 4) {
-        if (R == 4) { to_rt_kernel<T, 4><<<grid, 256, 0, st>>>(x, rt, du, dd, du_p, dd_p); return after_launch(m); }
+        if (R == 4) { to_rt_kernel<T, 4><<<grid, 256, 0, st>>>(x, rt, du, dd, du_p, dd_p, pu, pd); return after_launch(m); }
     }
-    if (R == 2) { to_rt_kernel<T, 2><<<grid, 256, 0, st>>>(x, rt, du, dd, du_p, dd_p); return after_launch(m); }
-    to_rt_kernel<T, 1><<<grid, 256, 0, st>>>(x, rt, du, dd, du_p, dd_p);
+    if (R == 2) { to_rt_kernel<T, 2><<<grid, 256, 0, st>>>(x, rt, du, dd, du_p, dd_p, pu, pd); return after_launch(m); }
+    to_rt_kernel<T, 1><<<grid, 256, 0, st>>>(x, rt, du, dd, du_p, dd_p, pu, pd);
     return after_launch(m);
 }
 
@@ -385,11 +391,12 @@ int launch_from_rt(hubbard_model *m, const T *rt, T *x, cudaStream_t st)
     const int R = gather_R(m);
     const int64_t du = m->up.dim, dd = m->dn.dim, du_p = round_up(du, R), dd_p = round_up(dd, R);
     const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((int64_t)m->sm_count * 8, (du_p / R * dd_p + 255) / 256));
+    const int32_t *pu = m->dev.gs_up.perm, *pd = m->dev.gs_dn.perm;
     if constexpr (sizeof(T) == 4) {
-        if (R == 4) { from_rt_kernel<T, 4><<<grid, 256, 0, st>>>(rt, x, du, dd, du_p, dd_p); return after_launch(m); }
+        if (R == 4) { from_rt_kernel<T, 4><<<grid, 256, 0, st>>>(rt, x, du, dd, du_p, dd_p, pu, pd); return after_launch(m); }
     }
-    if (R == 2) { from_rt_kernel<T, 2><<<grid, 256, 0, st>>>(rt, x, du, dd, du_p, dd_p); return after_launch(m); }
-    from_rt_kernel<T, 1><<<grid, 256, 0, st>>>(rt, x, du, dd, du_p, dd_p);
+    if (R == 2) { from_rt_kernel<T, 2><<<grid, 256, 0, st>>>(rt, x, du, dd, du_p, dd_p, pu, pd); return after_launch(m); }
+    from_rt_kernel<T, 1><<<grid, 256, 0, st>>>(rt, x, du, dd, du_p, dd_p, pu, pd);
     return after_launch(m);
 }
 
@@ -1141,20 +1148,25 @@ int hubbard_get_hops(const hubbard_model *m, int spin, int *width, int32_t *cols
     return HUBBARD_OK;
 }
 
-int hubbard_get_gather_table(const hubbard_model *m, int spin, int lanes, int64_t zero_base, int *slots, int64_t *ld,
-                             uint32_t *entries_host, int32_t *counts_host, int64_t *conflicts)
+int hubbard_get_gather_table(const hubbard_model *m, int spin, int lanes, int R, int sorted, int *slots, int64_t *ld,
+                             uint32_t *entries_host, int32_t *counts_host, uint16_t *warp_slots_host, int32_t *perm_host,
+                             int64_t *conflicts, int64_t *wavefronts)
 {
     if (!m || (spin != 0 && spin != 1) || lanes < 0 || lanes > 32 || (lanes & (lanes - 1)) != 0) return HUBBARD_ERR_INVALID;
+    if (R != 1 && R != 2 && R != 4) return HUBBARD_ERR_INVALID;
     const SpinTable &tab = spin == 0 ? m->up : m->dn;
-    if (zero_base < tab.dim) return HUBBARD_ERR_INVALID;
     try {
         GatherTable T;
-        build_gather_table(tab, lanes, zero_base, T);
+        build_gather_table(tab, lanes, R, sorted != 0, T, sorted == 2 ? m->bonds.data() : nullptr,
+                           sorted == 2 ? (int)(m->bonds.size() / 2) : 0);
         if (slots) *slots = T.w;
         if (ld) *ld = T.ld;
         if (conflicts) *conflicts = T.conflicts;
+        if (wavefronts) *wavefronts = T.wavefronts;
         if (entries_host) std::memcpy(entries_host, T.ent.data(), T.ent.size() * sizeof(uint32_t));
         if (counts_host) std::memcpy(counts_host, T.cnt.data(), T.cnt.size() * sizeof(int32_t));
+        if (warp_slots_host) std::memcpy(warp_slots_host, T.wslots.data(), T.wslots.size() * sizeof(uint16_t));
+        if (perm_host) std::memcpy(perm_host, T.perm.data(), T.perm.size() * sizeof(int32_t));
     } catch (const std::bad_alloc &) {
         return HUBBARD_ERR_HOST_OOM;
     }
@@ -1167,6 +1179,8 @@ struct OptKey { const char *name; int hub::DebugOptions::*field; bool layout; in
 const OptKey kOptKeys[] = {
     {"gather_R", &hub::DebugOptions::gather_R, true, 0, 4},
     {"gather_nosched", &hub::DebugOptions::gather_nosched, true, 0, 1},
+    {"gather_nosort", &hub::DebugOptions::gather_nosort, true, 0, 1},
+    {"gather_nosymmetry", &hub::DebugOptions::gather_nosymmetry, true, 0, 1},
     {"gather_ctas", &hub::DebugOptions::gather_ctas, false, 1, 4},
     {"apply_pure_gather", &hub::DebugOptions::apply_pure_gather, false, 0, 1},
     {"twosweep_old_row", &hub::DebugOptions::twosweep_old_row, false, 0, 1},
@@ -1208,6 +1222,7 @@ int hubbard_debug_get(const hubbard_model *m, const char *key, int *value)
     // what the library resolved (read-only)
     if (!std::strcmp(key, "resolved_variant")) { *value = m->has_device ? resolve_variant(m) : m->variant; return HUBBARD_OK; }
     if (!std::strcmp(key, "resolved_gather_R")) { *value = m->gather_R; return HUBBARD_OK; }
+    if (!std::strcmp(key, "resolved_gather_symmetry")) { *value = m->gather_symmetry; return HUBBARD_OK; }
     if (!std::strcmp(key, "resolved_cluster_row")) { *value = m->cluster_row; return HUBBARD_OK; }
     if (!std::strcmp(key, "resolved_cluster_R")) { *value = m->cluster_R; return HUBBARD_OK; }
     if (!std::strcmp(key, "resolved_cluster_NC")) { *value = m->cluster_NC; return HUBBARD_OK; }

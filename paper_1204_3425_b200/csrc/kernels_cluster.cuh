@@ -83,8 +83,8 @@ row_cluster_kernel(ClusterRowArgs<T> A)
         for (int il = threadIdx.x; il < my_w; il += kClusterThreads) {
             const int i = my0 + il;
             const bool valid = il < my_n;
-            const int n = valid ? A.in.cnt[i] : 0;
-            const int nb = max(1, (n + kGatherBatch - 1) / kGatherBatch);
+            const int n = (int)A.in.wslots[i >> 5];        // slots every lane of this warp walks (my0 is a multiple of 32)
+            const int nb = (n + kGatherBatch - 1) / kGatherBatch;
             const uint32_t sd = valid ? A.in.st[i] : 0u;
             T yold[R];
 #pragma unroll

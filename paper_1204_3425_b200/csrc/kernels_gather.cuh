@@ -14,7 +14,14 @@
 // format, stored so that a warp reads them coalesced: batches
 // of 8 entries of one state are contiguous, batch kb of state i at
 // [(kb * ld + i) * 8]) is read once per R outputs.  Padding entries point at a
-// zero slot.
+// zero slot.  Every lane of a warp walks the same, EXACT number of slots (the
+// table's per-warp count, gather_tables.h), so the trip count is warp-uniform
+// and the last, partial batch is cut with uniform branches.
+//
+// "State i" below is a POSITION in the table's internal order of the spin's basis
+// (gather_tables.h: groups ordered by hop count so that a warp's rows have nearly
+// equal length); the Lanczos work vectors live in that order for both spins, the
+// caller's row-major vectors are converted at the start / end of a run.
 //
 // Work vectors live in HBM in two TILE-MAJOR layouts, so that every tile either
 // sweep stages is ONE contiguous block that is already its shared-memory image
@@ -71,7 +78,6 @@ struct GatherArgs {
     double *partials;
     double *alpha_out, *beta_out;
     int y_rowmajor;         // ROW sweep of hubbard_apply writes y row-major (no CT buffers): hybrid with the strip sweep
-    int cnt_in_smem;        // hop counts cached in shared memory behind the tile (they fit and are < 256)
 };
 
 template <typename T, int N>
@@ -232,6 +238,25 @@ __device__ __forceinline__ void stage_rowmajor(const T *__restrict__ x, Pack<T, 
     }
 }
 
+// The 8 entries of a batch as 32-bit values (register-resident, constant indices only).
+template <typename E>
+__device__ __forceinline__ void unpack_batch(const Pack<E, kGatherBatch> &pk, uint32_t (&e)[kGatherBatch])
+{
+#pragma unroll
+    for (int j = 0; j < kGatherBatch; ++j) e[j] = pk.v[j];
+}
+
+// acc += +-Xs[col] for one hop entry (Algorithms 2/3: sum += Ax * x[Aj])
+template <typename T, int R>
+__device__ __forceinline__ void hop(const unsigned char *xs_bytes, uint32_t e, T (&acc)[R])
+{
+    using PR = Pack<T, R>;
+    const PR v = *reinterpret_cast<const PR *>(xs_bytes + (e & ~1u) * (uint32_t)(sizeof(PR) / 2));
+    const T s = sign_one<T>(e);
+#pragma unroll
+    for (int r = 0; r < R; ++r) acc[r] = fma(s, v.v[r], acc[r]);
+}
+
 // ------------------------------------------------------------------ the sweep
 // T: storage/arithmetic type.  R: rows (ROW) and columns (COL) per tile.
 // E: hop entry type.  COL: which sweep.  LZ: Lanczos form.
@@ -281,12 +306,15 @@ gather_sweep_kernel(GatherArgs<T> A)
         for (int r = 0; r < R; ++r) z.v[r] = T(0);
         Xs[n_in_p + threadIdx.x] = z;                     // zero slots, one per bank group (padding entries)
     }
-    unsigned char *cnt_s = smem_raw + (size_t)(n_in_p + kZeroSlots) * sizeof(PR);
-    if (A.cnt_in_smem)
-        for (int i = threadIdx.x; i < n_in_w; i += nthr) cnt_s[i] = (i < n_in) ? (unsigned char)A.in.cnt[i] : 0;
+    uint16_t *wsl_s = reinterpret_cast<uint16_t *>(smem_raw + (size_t)(n_in_p + kZeroSlots) * sizeof(PR));
+    for (int i = threadIdx.x; i < n_in_w / 32; i += nthr) wsl_s[i] = A.in.wslots[i];   // slots per warp of positions
     double racc = 0.0;                                    // |w|^2 (ROW) or q.f (COL) partial
     const int64_t tile_bytes = (int64_t)n_in_p * (int64_t)sizeof(PR);
     const int n_it = (n_in_w + nthr - 1) / nthr;                // gather iterations per tile
+    // Position handled by this thread in iteration `it`: stripes of nthr positions, the warps of every other
+    // stripe mirrored, so that with positions ordered by descending hop count all warps get equal work.
+    const int wv = (int)(threadIdx.x >> 5), nwv = nthr >> 5, ln = (int)(threadIdx.x & 31);
+    auto pos_of = [&](int it_) { return (it_ * nwv + ((it_ & 1) ? nwv - 1 - wv : wv)) * 32 + ln; };
     const int64_t pf_slice = ((tile_bytes + n_it - 1) / n_it + 15) / 16 * 16;       // bytes of the next tile requested per iteration
     const bool pf_ok = (tile_bytes % 16) == 0;            // bulk prefetches need 16-byte aligned addresses and sizes
     // buffers written in the other sweep's layout
@@ -356,13 +384,14 @@ gather_sweep_kernel(GatherArgs<T> A)
 #pragma unroll
             for (int r = 0; r < R; ++r) so[r] = (o0 + r < du) ? A.st_out[o0 + r] : 0u;
         }
-        int it = 0;
-        // every state has >= 1 (padding) batch; the table has n_in_w batches per plane, a block may have more threads
-        EB pk = load_batch(reinterpret_cast<const EB *>(ent) + min((int)threadIdx.x, n_in_w - 1));
-        for (int i = threadIdx.x; i < n_in_w; i += nthr, ++it) {
+        // every position has >= 1 (padding) batch; the table has n_in_w batches per plane, a block may have more threads
+        EB pk = load_batch(reinterpret_cast<const EB *>(ent) + min(pos_of(0), n_in_w - 1));
+        for (int it = 0; it < n_it; ++it) {
+            const int i = pos_of(it);
+            if (i >= n_in_w) continue;                    // whole warps: a partly filled last stripe
             const bool valid = i < n_in;
             const bool inpad = i < n_in_p;
-            const int n = A.cnt_in_smem ? (int)cnt_s[i] : (valid ? A.in.cnt[i] : 0);
+            const int n = (int)wsl_s[i >> 5];                // warp-uniform, >= 1
             // operands of the epilogue: requested now, used after the gather
             uint32_t sd = 0u;
             PR z, f;
@@ -397,20 +426,38 @@ gather_sweep_kernel(GatherArgs<T> A)
 #pragma unroll
             for (int r = 0; r < R; ++r) acc[r] = T(0);
             // one batch of hop entries is always in flight: the next batch of this state, or the first
-            // batch of this thread's next state (a state without hops still walks one padding batch)
+            // batch of this thread's next state
             const EB *ep = reinterpret_cast<const EB *>(ent) + i;
-            const int nb = max(1, (n + kGatherBatch - 1) / kGatherBatch);
-            for (int b = 0; b < nb; ++b) {
-                const EB *np = (b + 1 < nb) ? ep + ld : reinterpret_cast<const EB *>(ent) + min(i + nthr, n_in_w - 1);
-                ep = np;
-                const EB nxt = load_batch(np);
+            const int nb = (n + kGatherBatch - 1) / kGatherBatch;
+            for (int b = 0; b + 1 < nb; ++b) {
+                ep += ld;
+                const EB nxt = load_batch(ep);
+                uint32_t e[kGatherBatch];
+                unpack_batch<E>(pk, e);
 #pragma unroll
-                for (int j = 0; j < kGatherBatch; ++j) {
-                    const uint32_t e = pk.v[j];
-                    const PR v = *reinterpret_cast<const PR *>(xs_bytes + (e & ~1u) * (uint32_t)(sizeof(PR) / 2));
-                    const T s = sign_one<T>(e);
+                for (int j = 0; j < kGatherBatch; ++j) hop<T, R>(xs_bytes, e[j], acc);
+                pk = nxt;
+            }
+            {
+                const EB nxt = load_batch(reinterpret_cast<const EB *>(ent) + min(pos_of(it + 1), n_in_w - 1));
+                uint32_t e[kGatherBatch];
+                unpack_batch<E>(pk, e);
+                const int rem = n - (nb - 1) * kGatherBatch;     // 1..8 entries in the last batch, warp-uniform
+                if (rem == kGatherBatch) {
 #pragma unroll
-                    for (int r = 0; r < R; ++r) acc[r] = fma(s, v.v[r], acc[r]);
+                    for (int j = 0; j < kGatherBatch; ++j) hop<T, R>(xs_bytes, e[j], acc);
+                } else {
+                    static_assert(kGatherBatch == 8, "the partial batch is cut as 4 + 2 + 1");
+                    if (rem & 4) {
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) { hop<T, R>(xs_bytes, e[j], acc); e[j] = e[j + 4]; }
+                    }
+                    if (rem & 2) {
+                        hop<T, R>(xs_bytes, e[0], acc);
+                        hop<T, R>(xs_bytes, e[1], acc);
+                        e[0] = e[2];
+                    }
+                    if (rem & 1) hop<T, R>(xs_bytes, e[0], acc);
                 }
                 pk = nxt;
             }
@@ -489,21 +536,24 @@ gather_sweep_kernel(GatherArgs<T> A)
     }
 }
 
-// Start of a run: the caller's row-major start vector into the RT layout
-// (zero padding included).  One thread per 16-byte piece.
+// Start of a run: the caller's row-major start vector (basis order of PAPER.md:63-71) into the RT layout in
+// the internal order of both spins (zero padding included).  One thread per 16-byte piece.
 template <typename T, int R>
 __global__ void __launch_bounds__(256)
-to_rt_kernel(const T *__restrict__ x, T *__restrict__ rt, int64_t du, int64_t dd, int64_t du_p, int64_t dd_p)
+to_rt_kernel(const T *__restrict__ x, T *__restrict__ rt, int64_t du, int64_t dd, int64_t du_p, int64_t dd_p,
+             const int32_t *__restrict__ perm_up, const int32_t *__restrict__ perm_dn)
 {
     using PR = Pack<T, R>;
     const int64_t n = du_p / R * dd_p;
     for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p < n; p += (int64_t)gridDim.x * blockDim.x) {
-        const int64_t tile = p / dd_p, b = p - tile * dd_p;
+        const int64_t tile = p / dd_p, bp = p - tile * dd_p;
+        const int64_t b = (bp < dd) ? perm_dn[bp] : -1;
         PR v;
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            const int64_t a = tile * R + r;
-            v.v[r] = (a < du && b < dd) ? x[a * dd + b] : T(0);
+            const int64_t ap = tile * R + r;
+            const int64_t a = (ap < du) ? perm_up[ap] : -1;
+            v.v[r] = (a >= 0 && b >= 0) ? x[a * dd + b] : T(0);
         }
         reinterpret_cast<PR *>(rt)[p] = v;
     }
@@ -532,20 +582,23 @@ lanczos_final_norm_kernel(const T *__restrict__ Q, const T *__restrict__ F, int6
     }
 }
 
-// The RT layout back into the caller's row-major layout (ground-state vector).
+// The RT layout (internal order) back into the caller's row-major layout (ground-state vector).
 template <typename T, int R>
 __global__ void __launch_bounds__(256)
-from_rt_kernel(const T *__restrict__ rt, T *__restrict__ x, int64_t du, int64_t dd, int64_t du_p, int64_t dd_p)
+from_rt_kernel(const T *__restrict__ rt, T *__restrict__ x, int64_t du, int64_t dd, int64_t du_p, int64_t dd_p,
+               const int32_t *__restrict__ perm_up, const int32_t *__restrict__ perm_dn)
 {
     using PR = Pack<T, R>;
     const int64_t n = du_p / R * dd_p;
     for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p < n; p += (int64_t)gridDim.x * blockDim.x) {
-        const int64_t tile = p / dd_p, b = p - tile * dd_p;
+        const int64_t tile = p / dd_p, bp = p - tile * dd_p;
+        const int64_t b = (bp < dd) ? perm_dn[bp] : -1;
         const PR v = reinterpret_cast<const PR *>(rt)[p];
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            const int64_t a = tile * R + r;
-            if (a < du && b < dd) x[a * dd + b] = v.v[r];
+            const int64_t ap = tile * R + r;
+            const int64_t a = (ap < du) ? perm_up[ap] : -1;
+            if (a >= 0 && b >= 0) x[a * dd + b] = v.v[r];
         }
     }
 }

@@ -30,18 +30,21 @@ struct LanczosScalars {
     int started; // norm-producing sweeps finished (variant GATHER)
 };
 
-// One spin's hop table in the device layout of this variant: column-major ELL
-// [w][ld], entry = col * 2 + neg, the matrix element being t * (neg ? -1 : +1)
-// (PAPER.md:99-104); padding entries are dim * 2 (the zero slot, sign +).
+// One spin's hop table in the device layout of variant GATHER (gather_tables.h): batch-interleaved ELL over the
+// table's INTERNAL order of the basis states (position p <-> state perm[p]), entry = target_position * 2 + neg,
+// the matrix element being t * (neg ? -1 : +1); padding entries are (n_pos + z) * 2 (the zero
+// slots of the staged tile, sign +).
 struct SpinDev {
-    int64_t dim;            // dim_sigma
-    int64_t ld;             // states per batch plane (multiple of 32): entry k of state i
-                            // sits at [((k / 8) * ld + i) * 8 + k % 8]
-    int w;                  // ELL width rounded up to a multiple of 8
-    const uint16_t *e16;    // entries when dim + 1 <= 32768, else null
+    int64_t dim;            // dim_sigma (real states; positions >= dim are padding)
+    int64_t n_pos;          // positions of a staged tile: dim rounded up to the tile height R
+    int64_t ld;             // positions per batch plane (multiple of 32): entry k of position p
+                            // sits at [((k / 8) * ld + p) * 8 + k % 8]
+    int w;                  // slots per position in the table (multiple of 8)
+    const uint16_t *e16;    // entries when n_pos + 128 <= 32768, else null
     const uint32_t *e32;    // entries (always present)
-    const int32_t *cnt;     // hops per state
-    const uint32_t *st;     // basis bit patterns
+    const uint16_t *wslots; // per warp of 32 positions: slots every lane of that warp walks (exact)
+    const int32_t *perm;    // position -> state index in the basis order of PAPER.md:63-67 (-1: padding)
+    const uint32_t *st;     // basis bit patterns in position order (0 for padding)
 };
 
 // Everything a kernel needs to know about the model (passed by value).
@@ -59,7 +62,8 @@ struct DevModel {
     int w_dn;
     int64_t ld_dn;
     double t, U;
-    SpinDev g_up, g_dn;                  // tables of variant GATHER
+    SpinDev g_up, g_dn;                  // tables of variant GATHER in basis order (row-major callers: hubbard_apply)
+    SpinDev gs_up, gs_dn;                // the same in the sorted internal order of the Lanczos work vectors
 };
 
 struct ProfRecord {
@@ -72,6 +76,8 @@ struct ProfRecord {
 struct DebugOptions {
     int gather_R = 0;               // cap on the tile height R of variant GATHER (0 = none)
     int gather_nosched = 0;         // 1: hop entries in bond order, no bank-aware placement
+    int gather_nosort = 0;          // 1: the Lanczos work vectors keep the basis order (no internal reordering)
+    int gather_nosymmetry = 0;      // 1: internal order from hop counts only (no lattice-symmetry orbits)
     int gather_ctas = 4;            // CTAs per SM for small tiles
     int apply_pure_gather = 0;      // 1: plain hubbard_apply as two gather sweeps instead of the hybrid
     int twosweep_old_row = 0;       // 1: TWOSWEEP fallback keeps the first row kernel
@@ -103,6 +109,7 @@ struct hubbard_model {
     int cluster_row = 0;               // rows go through clusters (kernels_cluster.cuh): gather_R == 0 but a cluster holds them
     int cluster_R = 0, cluster_NC = 0, cluster_part = 0;
     int gather_R = 0;                  // tile height of variant GATHER, 0 = does not fit
+    int gather_symmetry = 0;           // order of the lattice symmetry group behind the internal order (0: none)
     hub::DebugOptions opt;
     std::vector<void *> layout_allocs;  // device tables that depend on `opt` (rebuilt by hubbard_debug_set)
 

@@ -151,49 +151,78 @@ def test_ground_energy_vs_lapack():
         hb.lanczos_ground_energy([float("nan")], [0.0], 1)
 
 
-@pytest.mark.parametrize("lanes", [0, 8, 16, 32])
+@pytest.mark.parametrize("sorted_", [0, 1, 2])
+@pytest.mark.parametrize("lanes,R", [(0, 1), (8, 2), (16, 1), (32, 1), (8, 4)])
 @pytest.mark.parametrize("name,ns,nu,nd,bonds", [
     ("C4", 16, 8, 8, torus_bonds(4, 4)), ("C2", 12, 6, 6, ring_bonds(12)), ("odd", 7, 3, 4, ring_bonds(7) + [(0, 3), (2, 6)]),
     ("dup", 6, 3, 3, ring_bonds(6) + [(0, 1)])])
-def test_gather_table_is_a_bank_aware_permutation_of_the_hops(name, ns, nu, nd, bonds, lanes):
-    """The device table of variant GATHER (host computation): per state the same
-    multiset of (column, sign) as the canonical hop list (duplicates kept as
-    separate entries), padding only beyond the sector, counts cover every real
-    entry, and - with scheduling on - (almost) no two lanes of a shared-memory
-    wavefront on one bank."""
+def test_gather_table_is_a_bank_aware_permutation_of_the_hops(name, ns, nu, nd, bonds, lanes, R, sorted_):
+    """The device table of variant GATHER (host computation): `perm` is a permutation of the basis states; per
+    position the same multiset of (column, sign) as the canonical hop list of its state, columns mapped through
+    the inverse permutation (duplicates kept as separate entries); every slot below the warp's exact count holds
+    a real entry or a zero slot beyond the tile; counts cover every real entry; and - with scheduling on - the
+    lanes of a shared-memory wavefront hit distinct banks up to the reported conflicts."""
     m = hb.hubbard_create_host(ns, nu, nd, bonds, 1.0, 0.0)
     ref = RefModel(ns, nu, nd, bonds, 1.0, 0.0)
     for spin in (0, 1):
         n = m.dim_up if spin == 0 else m.dim_dn
-        zero_base = (n + 1) // 2 * 2
-        w, ld, ent, cnt, conflicts = m.hubbard_get_gather_table(spin, lanes, zero_base)
-        assert w % 8 == 0 and ld % 32 == 0 and ld >= n
-        flat = ent.transpose(1, 0, 2).reshape(ld, w)            # [state][slot]
+        n_pos = (n + R - 1) // R * R
+        g = m.hubbard_get_gather_table(spin, lanes, R, sorted_)
+        w, ld, cnt, wsl, perm = g["slots"], g["ld"], g["counts"], g["warp_slots"], g["perm"]
+        assert w % 8 == 0 and ld % 32 == 0 and ld >= n_pos and len(wsl) == ld // 32
+        assert sorted(perm[:n]) == list(range(n)) and np.all(perm[n:] == -1)
+        if not sorted_ or lanes == 0:
+            if not sorted_:
+                assert np.array_equal(perm[:n], np.arange(n))
+        pos = np.empty(n, dtype=np.int64)
+        pos[perm[:n]] = np.arange(n)
+        flat = g["entries"].transpose(1, 0, 2).reshape(ld, w)            # [position][slot]
         rows = ref.hop_rows(spin)
         n_real = 0
-        for i in range(n):
-            e = flat[i, :cnt[i]]
-            real = e[(e >> 1) < n]
-            assert np.all((flat[i, cnt[i]:] >> 1) >= zero_base)                 # beyond the count: padding only
-            assert np.all((e[(e >> 1) >= n] >> 1) >= zero_base)
+        assert w >= int(wsl.max()) >= 1
+        for p in range(ld):
+            W = int(wsl[p // 32])
+            e = flat[p, :W]
+            assert cnt[p] <= W
+            real = e[(e >> 1) < n_pos]
+            assert np.all((e[(e >> 1) >= n_pos] >> 1) < n_pos + max(lanes, 1))   # zero slots of the tile
+            assert np.all((flat[p, cnt[p]:W] >> 1) >= n_pos)                     # beyond the count: padding only
+            if p >= n:
+                assert len(real) == 0
+                continue
             got = {}
             for x in real:                                                      # merge duplicates like the canonical form
                 got[int(x >> 1)] = got.get(int(x >> 1), 0.0) + (-1.0 if x & 1 else 1.0)
-            assert {c: v for c, v in got.items() if v != 0.0} == {c: v for c, v in rows[i]}
+            want = {int(pos[c]): v for c, v in rows[perm[p]]}
+            assert {c: v for c, v in got.items() if v != 0.0} == want
             n_real += len(real)
+        if sorted_ == 2 and lanes == 8 and name == "C4":
+            # the 4x4 torus has a translation group of 8 elements: almost all states sit in full orbits, the gather
+            # costs within 3 % of the ideal sum(hops) / lanes wavefronts and almost nothing collides
+            ideal = sum(len(r) for r in rows) / lanes
+            assert g["wavefronts"] <= 1.03 * ideal and g["conflicts"] <= n // 10
+        if sorted_ == 1 and lanes:
+            hops = np.array([sum(1 for _ in rows[perm[p]]) for p in range(n)])
+            gmax = [hops[g0:g0 + lanes].max() for g0 in range(0, n - n % lanes, lanes)]
+            if name != "dup":                                                    # (merged duplicates change the count)
+                assert all(a >= b for a, b in zip(gmax, gmax[1:]))              # groups ordered by their longest row
         if lanes:
-            # wavefront groups of `lanes` consecutive states: distinct banks per slot, up to the reported conflicts
+            # wavefront groups of `lanes` consecutive positions: distinct banks per slot, up to the reported conflicts
             worst = 0
-            for g0 in range(0, n, lanes):
-                blk = flat[g0:min(n, g0 + lanes)]
-                for s in range(w):
-                    col = blk[:, s] >> 1
-                    used = col[np.arange(len(blk)) + g0 < n]
-                    used = used[[s < cnt[g0 + k] for k in range(len(used))]]
-                    banks = used % lanes
+            for g0 in range(0, ld, lanes):
+                W = int(wsl[g0 // 32])
+                blk = flat[g0:g0 + lanes, :W] >> 1
+                for s in range(W):
+                    col = blk[:, s]
+                    banks = col[col < n_pos] % lanes
                     worst += len(banks) - len(np.unique(banks))
-            assert worst <= conflicts
-            assert conflicts <= max(4, n_real // 200)
+                    zb = col[col >= n_pos] % lanes                              # a zero slot never shares a bank with a real entry
+                    assert not set(zb.tolist()) & set(banks.tolist()) or len(np.unique(banks)) == lanes
+            assert worst <= g["conflicts"]
+            # the wavefront model: never worse than walking every warp's longest row rounded up to a batch
+            per_slot = 32 // lanes
+            old_cost = sum(-(-max(int(cnt[w0:w0 + 32].max()), 1) // 8) * 8 * per_slot for w0 in range(0, ld, 32))
+            assert g["wavefronts"] <= old_cost
 
 
 def test_ground_vector_vs_lapack():
