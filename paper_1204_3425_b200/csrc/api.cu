@@ -44,6 +44,7 @@ int dev_upload(hubbard_model *m, const std::vector<U> &h, const U **out, bool la
 }
 
 size_t elem_size(const hubbard_model *m) { return m->dtype == HUBBARD_F32 ? 4 : 8; }
+int64_t gather_align(const hubbard_model *m);
 int64_t model_dim(const hubbard_model *m) { return m->up.dim * m->dn.dim; }
 
 int build_host(hubbard_model **out, int n_sites, int n_up, int n_dn, const int32_t *bonds, int n_bonds,
@@ -84,7 +85,9 @@ int gather_R_for(const hubbard_model *m)
     const int forced = m->opt.gather_R;
     for (int R = (int)(16 / es); R >= 1; R >>= 1) {
         if (forced > 0 && R > forced) continue;
-        if ((size_t)(n_in + R + 128 / (R * es)) * R * es <= budget) return R;
+        // tile + zero slots + per-warp slot counts (2 bytes per 32 positions)
+        // tile (positions padded to R) + zero slots + per-warp slot counts (2 bytes per 32 positions)
+        if ((size_t)(n_in + R + 128 / (R * es)) * R * es + (size_t)(n_in + R + 32) / 32 * 2 + 16 <= budget) return R;
     }
     return 0;
 }
@@ -116,14 +119,15 @@ bool cluster_row_config(const hubbard_model *m, int *R_out, int *NC_out, int *pa
 }
 
 // Hop table of one spin for variant GATHER (kernels_gather.cuh, gather_tables.h).
-int upload_gather_table(hubbard_model *m, const SpinTable &tab, int R, bool sorted, SpinDev *out)
+// `align`: the tile's positions (and with them the zero slots padding entries point at) start at dim rounded up to it
+int upload_gather_table(hubbard_model *m, const SpinTable &tab, int R, int align, bool sorted, SpinDev *out)
 {
     SpinDev G{};
     const int es = m->dtype == HUBBARD_F32 ? 4 : 8;
     const int lanes = m->opt.gather_nosched ? 0 : 128 / (R * es);
     GatherTable T;
     const bool sym = sorted && !m->opt.gather_nosymmetry;
-    build_gather_table(tab, lanes, R, sorted && !m->opt.gather_nosort, T, sym ? m->bonds.data() : nullptr,
+    build_gather_table(tab, lanes, align, sorted && !m->opt.gather_nosort, T, sym ? m->bonds.data() : nullptr,
                        sym ? (int)(m->bonds.size() / 2) : 0);
     if (sorted) m->gather_symmetry = T.symmetry_order;
     G.dim = tab.dim; G.n_pos = T.n_pos; G.ld = T.ld; G.w = T.w;
@@ -158,13 +162,14 @@ int upload_layout_tables(hubbard_model *m)
         // variant GATHER: both spins column-major, entry = col * 2 + neg
         m->gather_R = gather_R_for(m);
         if (m->gather_R > 0) {
-            if ((rc = upload_gather_table(m, m->up, m->gather_R, false, &D.g_up))) return rc;
-            if ((rc = upload_gather_table(m, m->dn, m->gather_R, false, &D.g_dn))) return rc;
-            if ((rc = upload_gather_table(m, m->up, m->gather_R, true, &D.gs_up))) return rc;
-            if ((rc = upload_gather_table(m, m->dn, m->gather_R, true, &D.gs_dn))) return rc;
+            const int al = (int)gather_align(m);
+            if ((rc = upload_gather_table(m, m->up, m->gather_R, al, false, &D.g_up))) return rc;
+            if ((rc = upload_gather_table(m, m->dn, m->gather_R, al, false, &D.g_dn))) return rc;
+            if ((rc = upload_gather_table(m, m->up, m->gather_R, al, true, &D.gs_up))) return rc;
+            if ((rc = upload_gather_table(m, m->dn, m->gather_R, al, true, &D.gs_dn))) return rc;
         } else if (cluster_row_config(m, &m->cluster_R, &m->cluster_NC, &m->cluster_part)) {
             // R rows fit the shared memory of a cluster: down-spin table in that layout for kernels_cluster.cuh
-            if ((rc = upload_gather_table(m, m->dn, m->cluster_R, false, &D.g_dn))) return rc;
+            if ((rc = upload_gather_table(m, m->dn, m->cluster_R, m->cluster_R, false, &D.g_dn))) return rc;
             m->cluster_row = 1;
         }
     } catch (const std::bad_alloc &) {
@@ -302,10 +307,12 @@ bool gather_fits(const hubbard_model *m) { return gather_R(m) > 0; }
 int64_t round_up(int64_t n, int64_t r) { return (n + r - 1) / r * r; }
 
 // elements of one work vector of variant GATHER (either tile-major layout)
+// both dimensions of the tile-major work vectors are padded to the tile height R
+int64_t gather_align(const hubbard_model *m) { return std::max(1, gather_R(m)); }
+
 int64_t gather_vec_elems(const hubbard_model *m)
 {
-    const int R = std::max(1, gather_R(m));
-    return round_up(m->up.dim, R) * round_up(m->dn.dim, R);
+    return round_up(m->up.dim, gather_align(m)) * round_up(m->dn.dim, gather_align(m));
 }
 
 int resolve_variant(const hubbard_model *m)
@@ -322,15 +329,20 @@ int resolve_variant(const hubbard_model *m)
 }
 
 // ---- variant GATHER
+// shared memory of a gather sweep: the staged tile + its zero slots, then the per-warp slot counts
+size_t gather_smem_bytes(int64_t n_in_p, int R, size_t es)
+{
+    return (size_t)(n_in_p + 128 / (R * es)) * R * es + (size_t)(round_up(n_in_p, 32) / 32) * sizeof(uint16_t);
+}
+
 template <typename T, int R, typename E, bool COL, bool LZ>
 int launch_gather_inst(hubbard_model *m, GatherArgs<T> A, cudaStream_t st)
 {
     auto kern = gather_sweep_kernel<T, R, E, COL, LZ>;
-    A.du_p = round_up(A.dim_up, R);
-    A.dd_p = round_up(A.dim_dn, R);
+    A.du_p = round_up(A.dim_up, gather_align(m));
+    A.dd_p = round_up(A.dim_dn, gather_align(m));
     const int64_t n_in_p = COL ? A.du_p : A.dd_p;
-    // the staged tile + its zero slots, then the per-warp slot counts
-    const size_t smem = (size_t)(n_in_p + 128 / (R * sizeof(T))) * R * sizeof(T) + (size_t)(round_up(n_in_p, 32) / 32) * sizeof(uint16_t);
+    const size_t smem = gather_smem_bytes(n_in_p, R, sizeof(T));
     if (int rc = ensure_smem(m, kern, smem, true)) return rc;
     const int64_t tiles = (COL ? A.dd_p : A.du_p) / R;
     // Small sectors: several CTAs per SM (their staging and gather phases overlap one another); the 64-register
@@ -374,7 +386,7 @@ template <typename T>
 int launch_to_rt(hubbard_model *m, const T *x, T *rt, cudaStream_t st)
 {
     const int R = gather_R(m);
-    const int64_t du = m->up.dim, dd = m->dn.dim, du_p = round_up(du, R), dd_p = round_up(dd, R);
+    const int64_t du = m->up.dim, dd = m->dn.dim, du_p = round_up(du, gather_align(m)), dd_p = round_up(dd, gather_align(m));
     const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((int64_t)m->sm_count * 8, (du_p / R * dd_p + 255) / 256));
     const int32_t *pu = m->dev.gs_up.perm, *pd = m->dev.gs_dn.perm;
     if constexpr (sizeof(T) == 4) {
@@ -389,7 +401,7 @@ template <typename T>
 int launch_from_rt(hubbard_model *m, const T *rt, T *x, cudaStream_t st)
 {
     const int R = gather_R(m);
-    const int64_t du = m->up.dim, dd = m->dn.dim, du_p = round_up(du, R), dd_p = round_up(dd, R);
+    const int64_t du = m->up.dim, dd = m->dn.dim, du_p = round_up(du, gather_align(m)), dd_p = round_up(dd, gather_align(m));
     const int grid = (int)std::max<int64_t>(1, std::min<int64_t>((int64_t)m->sm_count * 8, (du_p / R * dd_p + 255) / 256));
     const int32_t *pu = m->dev.gs_up.perm, *pd = m->dev.gs_dn.perm;
     if constexpr (sizeof(T) == 4) {

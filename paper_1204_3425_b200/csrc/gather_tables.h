@@ -16,7 +16,7 @@ constexpr int kSlotBatch = GS_BATCH;   // == kGatherBatch of the kernels
 
 struct GatherTable {
     int64_t dim = 0;                // real states of the spin sector
-    int64_t n_pos = 0;              // internal positions: dim rounded up to the tile height R (the tail is padding)
+    int64_t n_pos = 0;              // internal positions: dim rounded up to `align` (the tail is padding)
     int64_t ld = 0;                 // positions per batch plane (n_pos rounded up to 32)
     int w = 0;                      // slots per position in the table (multiple of kSlotBatch, >= every warp's count)
     std::vector<uint32_t> ent;      // [(k / 8) * ld + p] * 8 + k % 8 : target_position * 2 + neg
@@ -33,7 +33,8 @@ struct GatherTable {
 // `lanes` = lanes served by one shared-memory wavefront of the gather (128 bytes /
 // bytes per staged element group: 8 for 16-byte groups, 16 for 8, 32 for 4); with
 // lanes == 0 the entries keep the order of `tab` (no scheduling).  The zero slots
-// of the staged tile (padding entries point at them) start at position n_pos.
+// of the staged tile (padding entries point at them) start at position n_pos =
+// dim rounded up to `align` (the kernels pad a tile to one 128-byte line of pieces).
 //
 // sorted: the internal order is chosen for the gather (below); otherwise it is
 // the basis order itself (perm = identity), which hubbard_apply's row-major
@@ -59,7 +60,7 @@ struct GatherTable {
 // banks) so that two entries of one slot do not hit the same bank.  W is chosen
 // per warp to minimise its wavefronts: one more slot costs 32 / lanes wavefronts,
 // one conflict costs one.
-void build_gather_table(const SpinTable &tab, int lanes, int R, bool sorted, GatherTable &out,
+void build_gather_table(const SpinTable &tab, int lanes, int align, bool sorted, GatherTable &out,
                         const int32_t *bonds = nullptr, int n_bonds = 0);
 
 }  // namespace hub

@@ -23,15 +23,18 @@
 // equal length); the Lanczos work vectors live in that order for both spins, the
 // caller's row-major vectors are converted at the start / end of a run.
 //
-// Work vectors live in HBM in two TILE-MAJOR layouts, so that every tile either
-// sweep stages is ONE contiguous block that is already its shared-memory image
-// (du_p, dd_p = dim_up, dim_dn rounded up to R; padding holds zeros):
-//   RT  (row tiles)     element (a, b) at ((a / R) * dd_p + b) * R + a % R
-//   CT  (column tiles)  element (a, b) at ((b / R) * du_p + a) * R + b % R
+// Work vectors live in HBM in two TILE-MAJOR layouts made of 16-byte PIECES (the R
+// values of one contracted position of one tile = one shared-memory slot), so
+// that every tile either sweep stages is ONE contiguous block that is already its
+// shared-memory image (du_p, dd_p = dim_up, dim_dn rounded up to R; padding holds
+// zeros):
+//   RT  piece (row tile m, column b)  at m * dd_p + b     element (a, b) at ((a / R) * dd_p + b) * R + a % R
+//   CT  piece (column tile c, row a)  at c * du_p + a     element (a, b) at ((b / R) * du_p + a) * R + b % R
 // A sweep reads its own layout contiguously and writes what the other sweep
 // will stage in the OTHER layout: the R x R block held by R adjacent lanes is
-// transposed with warp shuffles and each lane stores one 16-byte piece (full
-// 32/64-byte sectors, asynchronous) - all strided traffic is writes.
+// transposed with warp shuffles and each lane stores one piece (full 32/64-byte
+// sectors, asynchronous) - all strided traffic is writes (struct Layout records
+// what interleaving several tiles line by line did instead).
 //
 // Lanczos form (Algorithm 1 with eq. 13), no separate
 // axpy/norm kernel:
@@ -83,6 +86,21 @@ struct GatherArgs {
 template <typename T, int N>
 struct alignas(sizeof(T) * N) Pack {
     T v[N];
+};
+
+// Piece index of (tile, position) in a tile-major layout whose contracted dimension has n_p positions.
+// S tiles can be interleaved line by line into a super-tile (S = 1: every tile is one contiguous block).  Measured
+// on C4 fp64: S = 4 turns the transposed 32-byte stores into whole 128-byte lines, which HBM
+// takes at 4.6 instead of 2.9 TB/s in isolation, but the tile is then READ as sectors at a 128-byte stride - four
+// times the lines per load instruction, and the sweeps are bound by load latency: 5.0 ms per iteration against 3.6
+// (S = 2: 4.0 ms).  S = 1 it is.
+template <typename T, int R>
+struct Layout {
+    static constexpr int S = 1;
+    static __host__ __device__ __forceinline__ int64_t piece(int64_t tile, int64_t pos, int64_t n_p)
+    {
+        return (((tile / S) * (n_p / R) + pos / R) * S + tile % S) * R + pos % R;
+    }
 };
 
 template <typename T> __device__ __forceinline__ T sign_one(uint32_t e);
@@ -204,6 +222,13 @@ __device__ __forceinline__ Pack<T, R> block_transpose(const T (&v)[R], int q)
         o.v[0] = v[0];
         return o;
     }
+    if constexpr (R == 2) {
+        // lane q keeps element q of its own column and swaps the other one with its partner
+        const T got = __shfl_xor_sync(0xffffffffu, q ? v[0] : v[1], 1);
+        o.v[0] = q ? got : v[0];
+        o.v[1] = q ? v[1] : got;
+        return o;
+    }
     T tmp[R];
     tmp[0] = pick<T, R>(v, q);
 #pragma unroll
@@ -238,14 +263,6 @@ __device__ __forceinline__ void stage_rowmajor(const T *__restrict__ x, Pack<T, 
     }
 }
 
-// The 8 entries of a batch as 32-bit values (register-resident, constant indices only).
-template <typename E>
-__device__ __forceinline__ void unpack_batch(const Pack<E, kGatherBatch> &pk, uint32_t (&e)[kGatherBatch])
-{
-#pragma unroll
-    for (int j = 0; j < kGatherBatch; ++j) e[j] = pk.v[j];
-}
-
 // acc += +-Xs[col] for one hop entry (Algorithms 2/3: sum += Ax * x[Aj])
 template <typename T, int R>
 __device__ __forceinline__ void hop(const unsigned char *xs_bytes, uint32_t e, T (&acc)[R])
@@ -255,6 +272,75 @@ __device__ __forceinline__ void hop(const unsigned char *xs_bytes, uint32_t e, T
     const T s = sign_one<T>(e);
 #pragma unroll
     for (int r = 0; r < R; ++r) acc[r] = fma(s, v.v[r], acc[r]);
+}
+
+// ---- hop entries straight from the packed 32-bit words of a batch (uint16 entries: two per word), without
+// unpacking them first: byte offset of entry e = (e & ~1) * sizeof(PR) / 2, sign = bit 0.
+template <typename T, int R>
+__device__ __forceinline__ void hop_lo(const unsigned char *xs_bytes, uint32_t w, T (&acc)[R])      // entry in bits 0..15
+{
+    using PR = Pack<T, R>;
+    constexpr int SH = sizeof(PR) == 16 ? 3 : sizeof(PR) == 8 ? 2 : 1;
+    const PR v = *reinterpret_cast<const PR *>(xs_bytes + ((w << SH) & (0xfffeu << SH)));
+    const T s = sign_one<T>(w);                            // (w << 31): only bit 0 survives
+#pragma unroll
+    for (int r = 0; r < R; ++r) acc[r] = fma(s, v.v[r], acc[r]);
+}
+template <typename T, int R>
+__device__ __forceinline__ void hop_hi(const unsigned char *xs_bytes, uint32_t w, T (&acc)[R])      // entry in bits 16..31
+{
+    using PR = Pack<T, R>;
+    constexpr int SH = sizeof(PR) == 16 ? 3 : sizeof(PR) == 8 ? 2 : 1;
+    const PR v = *reinterpret_cast<const PR *>(xs_bytes + ((w >> (16 - SH)) & (0xfffeu << SH)));
+    const T s = sign_one<T>(w >> 16);
+#pragma unroll
+    for (int r = 0; r < R; ++r) acc[r] = fma(s, v.v[r], acc[r]);
+}
+
+// `count` (warp-uniform, 1..8) entries of a batch.
+template <typename T, int R>
+__device__ __forceinline__ void hop_batch_n(const unsigned char *xs_bytes, const Pack<uint16_t, kGatherBatch> &pk, int count, T (&acc)[R])
+{
+    static_assert(kGatherBatch == 8, "a batch is four 32-bit words of two entries");
+    uint32_t w[4];
+    memcpy(w, &pk, 16);
+    if (count == kGatherBatch) {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) { hop_lo<T, R>(xs_bytes, w[k], acc); hop_hi<T, R>(xs_bytes, w[k], acc); }
+    } else {
+        if (count & 4) {
+            hop_lo<T, R>(xs_bytes, w[0], acc); hop_hi<T, R>(xs_bytes, w[0], acc);
+            hop_lo<T, R>(xs_bytes, w[1], acc); hop_hi<T, R>(xs_bytes, w[1], acc);
+            w[0] = w[2]; w[1] = w[3];
+        }
+        if (count & 2) {
+            hop_lo<T, R>(xs_bytes, w[0], acc); hop_hi<T, R>(xs_bytes, w[0], acc);
+            w[0] = w[1];
+        }
+        if (count & 1) hop_lo<T, R>(xs_bytes, w[0], acc);
+    }
+}
+template <typename T, int R>
+__device__ __forceinline__ void hop_batch_n(const unsigned char *xs_bytes, const Pack<uint32_t, kGatherBatch> &pk, int count, T (&acc)[R])
+{
+    uint32_t e[kGatherBatch];
+#pragma unroll
+    for (int j = 0; j < kGatherBatch; ++j) e[j] = pk.v[j];
+    if (count == kGatherBatch) {
+#pragma unroll
+        for (int j = 0; j < kGatherBatch; ++j) hop<T, R>(xs_bytes, e[j], acc);
+    } else {
+        if (count & 4) {
+#pragma unroll
+            for (int j = 0; j < 4; ++j) { hop<T, R>(xs_bytes, e[j], acc); e[j] = e[j + 4]; }
+        }
+        if (count & 2) {
+            hop<T, R>(xs_bytes, e[0], acc);
+            hop<T, R>(xs_bytes, e[1], acc);
+            e[0] = e[2];
+        }
+        if (count & 1) hop<T, R>(xs_bytes, e[0], acc);
+    }
 }
 
 // ------------------------------------------------------------------ the sweep
@@ -321,23 +407,29 @@ gather_sweep_kernel(GatherArgs<T> A)
     PR *outW = reinterpret_cast<PR *>(A.Wct);             // ROW: w (or x) in CT
     PR *outZ = reinterpret_cast<PR *>(COL ? A.Frt : A.Zct);   // ROW: z in CT;  COL/LZ: q in RT
 
+    using LY = Layout<T, R>;
+    constexpr int S = LY::S;
+    // piece of position i of the current tile
+    auto poff = [&](int i) { return (int64_t)(i / R) * (S * R) + i % R; };
+
     for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
         const int64_t o0 = tile * R;
+        const int64_t tbase = LY::piece(tile, 0, n_in_p);
         __syncthreads();                                  // gathers of the previous tile are done
         // ---- stage the tile
         if (COL || LZ) {
-            // tile-major layouts: the tile is one contiguous block, already interleaved
-            const PR *src = reinterpret_cast<const PR *>(COL ? A.Wct : A.Qrt) + tile * n_in_p;
+            // tile-major layouts: the pieces are already the interleaved shared-memory image
+            const PR *src = reinterpret_cast<const PR *>(COL ? A.Wct : A.Qrt) + tbase;
             if (!COL) {
-                const PR *fsrc = reinterpret_cast<const PR *>(A.Frt) + tile * n_in_p;
-                PR *wdst = reinterpret_cast<PR *>(A.Qrt) + tile * n_in_p;
+                const PR *fsrc = reinterpret_cast<const PR *>(A.Frt) + tbase;
+                PR *wdst = reinterpret_cast<PR *>(A.Qrt) + tbase;
                 // loads of kStageUnroll pieces are issued before the first store (w overwrites q in place)
                 for (int i0 = threadIdx.x; i0 < n_in_p; i0 += kStageUnroll * nthr) {
                     PR v[kStageUnroll], f[kStageUnroll];
 #pragma unroll
                     for (int u = 0; u < kStageUnroll; ++u) {
                         const int i = i0 + u * nthr;
-                        if (i < n_in_p) { v[u] = ld_once<1>(src + i); f[u] = ld_once<1>(fsrc + i); }
+                        if (i < n_in_p) { v[u] = ld_once<1>(src + poff(i)); f[u] = ld_once<1>(fsrc + poff(i)); }
                     }
 #pragma unroll
                     for (int u = 0; u < kStageUnroll; ++u) {
@@ -348,7 +440,7 @@ gather_sweep_kernel(GatherArgs<T> A)
                                 v[u].v[r] = v[u].v[r] - ac * f[u].v[r];
                                 racc += (double)v[u].v[r] * (double)v[u].v[r];
                             }
-                            st_once<1>(wdst + i, v[u]);
+                            st_once<1>(wdst + poff(i), v[u]);
                             Xs[i] = v[u];
                         }
                     }
@@ -359,7 +451,7 @@ gather_sweep_kernel(GatherArgs<T> A)
 #pragma unroll
                     for (int u = 0; u < kStageUnroll; ++u) {
                         const int i = i0 + u * nthr;
-                        if (i < n_in_p) v[u] = ld_once<2>(src + i);
+                        if (i < n_in_p) v[u] = ld_once<2>(src + poff(i));
                     }
 #pragma unroll
                     for (int u = 0; u < kStageUnroll; ++u) {
@@ -401,22 +493,24 @@ gather_sweep_kernel(GatherArgs<T> A)
             if (!COL) {
                 if (valid) sd = A.in.st[i];
             } else if (inpad) {
-                z = ld_once<(sizeof(T) == 4 ? 4 : 8)>(reinterpret_cast<const PR *>(A.Zct) + tile * n_in_p + i);
-                if (LZ) f = ld_once<(sizeof(T) == 4 ? 4 : 8)>(reinterpret_cast<const PR *>(A.Fct) + tile * n_in_p + i);
+                z = ld_once<(sizeof(T) == 4 ? 4 : 8)>(reinterpret_cast<const PR *>(A.Zct) + tbase + poff(i));
+                if (LZ) f = ld_once<(sizeof(T) == 4 ? 4 : 8)>(reinterpret_cast<const PR *>(A.Fct) + tbase + poff(i));
             }
 #endif
             // keep DRAM busy during the gather: a slice of the next tile's inputs goes to L2 every iteration
 #if GS_L2PF
+            // (the S tiles of a super-tile share one contiguous region of S * tile_bytes: each of their CTAs
+            // requests the S-th part of it that has its own number)
             if ((COL || LZ) && pf_ok && tile + gridDim.x < n_tiles) {
                 const int64_t off = (int64_t)it * pf_slice + (int64_t)threadIdx.x * 2048;
                 if (threadIdx.x * 2048 < pf_slice && off < tile_bytes) {
                     const unsigned nb = (unsigned)min((int64_t)2048, min(pf_slice - (int64_t)threadIdx.x * 2048, tile_bytes - off));
-                    const char *p0 = reinterpret_cast<const char *>(reinterpret_cast<const PR *>(COL ? A.Wct : A.Qrt) +
-                                                                    (tile + gridDim.x) * n_in_p) + off;
+                    const int64_t tn = tile + gridDim.x;
+                    const int64_t region = LY::piece(tn - tn % S, 0, n_in_p) + (tn % S) * (int64_t)n_in_p;    // in pieces
+                    const char *p0 = reinterpret_cast<const char *>(reinterpret_cast<const PR *>(COL ? A.Wct : A.Qrt) + region) + off;
                     asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p0), "r"(nb) : "memory");
                     if (!COL) {
-                        const char *p1 = reinterpret_cast<const char *>(reinterpret_cast<const PR *>(A.Frt) +
-                                                                        (tile + gridDim.x) * n_in_p) + off;
+                        const char *p1 = reinterpret_cast<const char *>(reinterpret_cast<const PR *>(A.Frt) + region) + off;
                         asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p1), "r"(nb) : "memory");
                     }
                 }
@@ -432,33 +526,12 @@ gather_sweep_kernel(GatherArgs<T> A)
             for (int b = 0; b + 1 < nb; ++b) {
                 ep += ld;
                 const EB nxt = load_batch(ep);
-                uint32_t e[kGatherBatch];
-                unpack_batch<E>(pk, e);
-#pragma unroll
-                for (int j = 0; j < kGatherBatch; ++j) hop<T, R>(xs_bytes, e[j], acc);
+                hop_batch_n<T, R>(xs_bytes, pk, kGatherBatch, acc);
                 pk = nxt;
             }
             {
                 const EB nxt = load_batch(reinterpret_cast<const EB *>(ent) + min(pos_of(it + 1), n_in_w - 1));
-                uint32_t e[kGatherBatch];
-                unpack_batch<E>(pk, e);
-                const int rem = n - (nb - 1) * kGatherBatch;     // 1..8 entries in the last batch, warp-uniform
-                if (rem == kGatherBatch) {
-#pragma unroll
-                    for (int j = 0; j < kGatherBatch; ++j) hop<T, R>(xs_bytes, e[j], acc);
-                } else {
-                    static_assert(kGatherBatch == 8, "the partial batch is cut as 4 + 2 + 1");
-                    if (rem & 4) {
-#pragma unroll
-                        for (int j = 0; j < 4; ++j) { hop<T, R>(xs_bytes, e[j], acc); e[j] = e[j + 4]; }
-                    }
-                    if (rem & 2) {
-                        hop<T, R>(xs_bytes, e[0], acc);
-                        hop<T, R>(xs_bytes, e[1], acc);
-                        e[0] = e[2];
-                    }
-                    if (rem & 1) hop<T, R>(xs_bytes, e[0], acc);
-                }
+                hop_batch_n<T, R>(xs_bytes, pk, n - (nb - 1) * kGatherBatch, acc);    // 1..8 entries, warp-uniform
                 pk = nxt;
             }
             PR xi;
@@ -469,12 +542,13 @@ gather_sweep_kernel(GatherArgs<T> A)
             if (!COL) {
                 if (valid) sd = A.in.st[i];
             } else if (inpad) {
-                z = ld_once<(sizeof(T) == 4 ? 4 : 8)>(reinterpret_cast<const PR *>(A.Zct) + tile * n_in_p + i);
-                if (LZ) f = ld_once<(sizeof(T) == 4 ? 4 : 8)>(reinterpret_cast<const PR *>(A.Fct) + tile * n_in_p + i);
+                z = ld_once<(sizeof(T) == 4 ? 4 : 8)>(reinterpret_cast<const PR *>(A.Zct) + tbase + poff(i));
+                if (LZ) f = ld_once<(sizeof(T) == 4 ? 4 : 8)>(reinterpret_cast<const PR *>(A.Fct) + tbase + poff(i));
             }
 #endif
             const int q = i % R;
-            const int64_t oidx = (int64_t)(i / R) * n_out_p + o0 + q;    // this lane's 16-byte piece in the other layout
+            // this lane's piece in the other layout (R adjacent lanes: one 32/64-byte sector)
+            const int64_t oidx = LY::piece(i / R, o0 + q, n_out_p);
             if (!COL) {
                 // Algorithm 4: on-the-fly diagonal
                 T h[R];
@@ -544,9 +618,12 @@ to_rt_kernel(const T *__restrict__ x, T *__restrict__ rt, int64_t du, int64_t dd
              const int32_t *__restrict__ perm_up, const int32_t *__restrict__ perm_dn)
 {
     using PR = Pack<T, R>;
+    constexpr int S = Layout<T, R>::S;
     const int64_t n = du_p / R * dd_p;
     for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p < n; p += (int64_t)gridDim.x * blockDim.x) {
-        const int64_t tile = p / dd_p, bp = p - tile * dd_p;
+        // piece p of the RT layout -> (row tile, column position)
+        const int64_t t1 = p / R, t2 = t1 / S;
+        const int64_t tile = (t2 / (dd_p / R)) * S + t1 % S, bp = (t2 % (dd_p / R)) * R + p % R;
         const int64_t b = (bp < dd) ? perm_dn[bp] : -1;
         PR v;
 #pragma unroll
@@ -589,9 +666,11 @@ from_rt_kernel(const T *__restrict__ rt, T *__restrict__ x, int64_t du, int64_t 
                const int32_t *__restrict__ perm_up, const int32_t *__restrict__ perm_dn)
 {
     using PR = Pack<T, R>;
+    constexpr int S = Layout<T, R>::S;
     const int64_t n = du_p / R * dd_p;
     for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p < n; p += (int64_t)gridDim.x * blockDim.x) {
-        const int64_t tile = p / dd_p, bp = p - tile * dd_p;
+        const int64_t t1 = p / R, t2 = t1 / S;
+        const int64_t tile = (t2 / (dd_p / R)) * S + t1 % S, bp = (t2 % (dd_p / R)) * R + p % R;
         const int64_t b = (bp < dd) ? perm_dn[bp] : -1;
         const PR v = reinterpret_cast<const PR *>(rt)[p];
 #pragma unroll
