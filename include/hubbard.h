@@ -172,9 +172,19 @@ int lanczos_ground_state(hubbard_model *m, const void *v0_dev, int iters, void *
  * for a REAL start vector v0 (tau: imaginary time, t: real time).  out_re_dev / out_im_dev: device, dim elements
  * of the model's dtype, row-major, caller-owned, distinct from v0 and from each other; out_im_dev may be NULL
  * (e.g. t == 0).  Pass 1 is lanczos_run, the host exponentiates T_m (full tridiagonal eigen-decomposition), each
- * output part is one more identical run accumulating sum_j y_j f_j.  Synchronises the stream. */
+ * output part is one more identical run accumulating sum_j y_j f_j.  Synchronises the stream.
+ * (v0 must differ from the outputs here; lanczos_propagate_complex allows in-place continuation.) */
 int lanczos_propagate(hubbard_model *m, const void *v0_dev, int iters, double tau, double t, void *out_re_dev,
                       void *out_im_dev, int *iters_done, void *stream);
+
+/* lanczos_propagate_complex: the same for a COMPLEX start vector psi = re_in + i im_in (im_in_dev may be NULL = 0), so
+ * that a propagation can be continued: out = exp(-(tau + i t) H) psi.  The output buffers may be the input buffers
+ * (in-place continuation), but out_re_dev != out_im_dev; both outputs are required.  H is real symmetric, so this is
+ * REAL Lanczos on the stacked vector [re ; im] with diag(H, H) and the real inner product - the library runs it as
+ * the same lattice with the up sector listed twice through the unchanged kernels (a second model of twice the size
+ * and three buffers of 2 * dim elements are allocated on first use and kept).  *iters_done as above.  Synchronises. */
+int lanczos_propagate_complex(hubbard_model *m, const void *re_in_dev, const void *im_in_dev, int iters, double tau, double t,
+                              void *out_re_dev, void *out_im_dev, int *iters_done, void *stream);
 
 /* Breakdown threshold tau (>= 0; 0 = the paper's literal "b = 0" test). */
 int lanczos_set_tau(hubbard_model *m, double tau);

@@ -20,7 +20,7 @@ KCLASS_NAMES = ("hv_paper", "row_sweep", "col_sweep", "vec_sweep", "scalar", "se
 ABI_SYMBOLS = (
     "hubbard_create", "hubbard_create_host", "hubbard_destroy", "hubbard_dims", "hubbard_set_U",
     "hubbard_set_variant", "hubbard_apply", "lanczos_run", "lanczos_run_until", "lanczos_ground_state",
-    "lanczos_ground_vector", "lanczos_propagate", "lanczos_expm_e1", "lanczos_set_tau", "hubbard_apply_host",
+    "lanczos_ground_vector", "lanczos_propagate", "lanczos_propagate_complex", "lanczos_expm_e1", "lanczos_set_tau", "hubbard_apply_host",
     "lanczos_run_host", "hubbard_get_basis", "hubbard_get_hops", "hubbard_get_gather_table", "lanczos_ground_energy",
     "hubbard_profile", "hubbard_kernel_times", "hubbard_launch_count", "hubbard_last_cuda_error",
     "hubbard_strerror", "hubbard_debug_set", "hubbard_debug_get",
@@ -51,6 +51,7 @@ def _load() -> C.CDLL:
     lib.lanczos_ground_state.argtypes = [vp, vp, i32, vp, P(dbl), P(i32), vp]
     lib.lanczos_ground_vector.argtypes = [P(dbl), P(dbl), i32, P(dbl), P(dbl)]
     lib.lanczos_propagate.argtypes = [vp, vp, i32, dbl, dbl, vp, vp, P(i32), vp]
+    lib.lanczos_propagate_complex.argtypes = [vp, vp, vp, i32, dbl, dbl, vp, vp, P(i32), vp]
     lib.lanczos_expm_e1.argtypes = [P(dbl), P(dbl), i32, dbl, dbl, P(dbl), P(dbl)]
     lib.hubbard_apply_host.argtypes = [vp, vp, vp, vp]
     lib.lanczos_run_host.argtypes = [vp, vp, i32, P(dbl), P(dbl), P(i32), vp]
@@ -202,6 +203,14 @@ class Model:
         _check(lib.lanczos_propagate(self._h, _dptr(v0), iters, float(tau), float(t), _dptr(out_re),
                                      _dptr(out_im) if out_im is not None else None, C.byref(done), _stream(stream)),
                "lanczos_propagate", self._h)
+        return done.value
+
+    def lanczos_propagate_complex(self, re_in, im_in, iters, tau, t, out_re, out_im, stream=None):
+        """(out_re + i out_im) = exp(-(tau + i t) H) (re_in + i im_in); im_in may be None; returns the iterations done."""
+        done = C.c_int(0)
+        _check(lib.lanczos_propagate_complex(self._h, _dptr(re_in), _dptr(im_in) if im_in is not None else None, iters,
+                                             float(tau), float(t), _dptr(out_re), _dptr(out_im), C.byref(done), _stream(stream)),
+               "lanczos_propagate_complex", self._h)
         return done.value
 
     # -- hot path, host buffers (numpy arrays or CPU torch tensors)

@@ -944,6 +944,78 @@ int lanczos_propagate_impl(hubbard_model *m, const T *v0, int iters, double tau,
     return HUBBARD_OK;
 }
 
+// ---- complex start vectors (second half): a propagated state is complex, psi = x + i y.  H is real
+// symmetric, so Lanczos on psi is REAL Lanczos on the stacked vector [x ; y] with the block-diagonal operator
+// diag(H, H) and the real inner product (the recurrence polynomials have real coefficients a_j, b_j, and
+// <p(H) psi, q(H) psi> is real for real polynomials).  diag(H, H) is this library's H for the same lattice with the
+// up sector listed twice: V becomes a (2 dim_up) x dim_dn matrix, H_up -> I_2 (x) H_up, the diagonal repeats.  The
+// "twin" model holds exactly that and runs through the unchanged kernels.
+int ensure_twin(hubbard_model *m)
+{
+    if (!m->twin) {
+        hubbard_model *t = new (std::nothrow) hubbard_model();
+        if (!t) return HUBBARD_ERR_HOST_OOM;
+        try {
+            t->n_sites = m->n_sites; t->n_up = m->n_up; t->n_dn = m->n_dn; t->dtype = m->dtype; t->t = m->t; t->U = m->U;
+            t->bonds = m->bonds;
+            t->dn = m->dn;
+            const SpinTable &u = m->up;
+            SpinTable &d = t->up;
+            d.n_sites = u.n_sites; d.n_el = u.n_el; d.dim = 2 * u.dim; d.width = u.width;
+            if (d.dim >= 0x7fffffffll) { delete t; return HUBBARD_ERR_UNSUPPORTED; }
+            d.states = u.states;
+            d.states.insert(d.states.end(), u.states.begin(), u.states.end());
+            d.col = u.col;
+            d.plus = u.plus;
+            d.rowptr = u.rowptr;
+            const int64_t nnz = u.rowptr[(size_t)u.dim];
+            for (int64_t r = 1; r <= u.dim; ++r) d.rowptr.push_back(nnz + u.rowptr[(size_t)r]);
+            for (int64_t k = 0; k < nnz; ++k) { d.col.push_back(u.col[(size_t)k] + (int32_t)u.dim); d.plus.push_back(u.plus[(size_t)k]); }
+        } catch (const std::bad_alloc &) {
+            delete t;
+            return HUBBARD_ERR_HOST_OOM;
+        }
+        t->opt = m->opt;
+        t->opt.gather_nosymmetry = 1;            // the orbit construction assumes distinct bit patterns
+        t->sm_count = m->sm_count; t->max_smem_optin = m->max_smem_optin; t->coop_launch = m->coop_launch;
+        int rc = upload_tables(t);
+        if (rc) { hubbard_destroy(t); return rc; }
+        t->has_device = true;
+        m->twin = t;
+    }
+    hubbard_model *t = m->twin;
+    t->U = m->U; t->dev.U = m->U; t->tau = m->tau;
+    t->variant = (m->variant == HUBBARD_VARIANT_GATHER && !gather_fits(t)) ? HUBBARD_VARIANT_AUTO : m->variant;
+    const size_t bytes = 2 * (size_t)model_dim(m) * elem_size(m);
+    for (int k = 0; k < 3; ++k)
+        if (!m->cplx[k]) CU_TRY(m, cudaMalloc(&m->cplx[k], std::max<size_t>(bytes, 16)));
+    return HUBBARD_OK;
+}
+
+template <typename T>
+int lanczos_propagate_complex_impl(hubbard_model *m, const T *re_in, const T *im_in, int iters, double tau, double t,
+                                   T *out_re, T *out_im, int *done, cudaStream_t st)
+{
+    int rc = ensure_twin(m);
+    if (rc) return rc;
+    hubbard_model *tw = m->twin;
+    const int64_t dim = model_dim(m);
+    T *v2 = static_cast<T *>(m->cplx[0]), *A = static_cast<T *>(m->cplx[1]), *B = static_cast<T *>(m->cplx[2]);
+    CU_TRY(m, cudaMemcpyAsync(v2, re_in, (size_t)dim * sizeof(T), cudaMemcpyDeviceToDevice, st));
+    if (im_in) CU_TRY(m, cudaMemcpyAsync(v2 + dim, im_in, (size_t)dim * sizeof(T), cudaMemcpyDeviceToDevice, st));
+    else CU_TRY(m, cudaMemsetAsync(v2 + dim, 0, (size_t)dim * sizeof(T), st));
+    // real Lanczos on [x ; y] with diag(H, H): the existing real propagation gives A = Re-coefficients, B = Im-coefficients
+    rc = lanczos_propagate_impl<T>(tw, v2, iters, tau, t, A, B, done, st);
+    m->last_cuda_error = tw->last_cuda_error;
+    m->launches += tw->launches; tw->launches = 0;
+    if (rc) return rc;
+    const int grid = lanczos_vec_grid(m, dim);
+    complex_mix_kernel<T><<<grid, kVecThreads, 0, st>>>(A, B, dim, out_re, out_im);
+    if ((rc = after_launch(m))) return rc;
+    CU_TRY(m, cudaStreamSynchronize(st));
+    return HUBBARD_OK;
+}
+
 int ensure_stage(hubbard_model *m, int which)
 {
     if (m->stage[which]) return HUBBARD_OK;
@@ -999,6 +1071,8 @@ void hubbard_destroy(hubbard_model *m)
     for (int i = 0; i < 6; ++i) if (m->work[i]) cudaFree(m->work[i]);
     if (m->d_ycoef) cudaFree(m->d_ycoef);
     for (int i = 0; i < 2; ++i) if (m->stage[i]) cudaFree(m->stage[i]);
+    for (int i = 0; i < 3; ++i) if (m->cplx[i]) cudaFree(m->cplx[i]);
+    if (m->twin) hubbard_destroy(m->twin);
     if (m->d_scal) cudaFree(m->d_scal);
     if (m->d_partial) cudaFree(m->d_partial);
     if (m->d_alpha) cudaFree(m->d_alpha);
@@ -1111,6 +1185,23 @@ int lanczos_propagate(hubbard_model *m, const void *v0_dev, int iters, double ta
                                              static_cast<float *>(out_im_dev), iters_done, st);
     return lanczos_propagate_impl<double>(m, static_cast<const double *>(v0_dev), iters, tau, t, static_cast<double *>(out_re_dev),
                                           static_cast<double *>(out_im_dev), iters_done, st);
+}
+
+int lanczos_propagate_complex(hubbard_model *m, const void *re_in_dev, const void *im_in_dev, int iters, double tau, double t,
+                              void *out_re_dev, void *out_im_dev, int *iters_done, void *stream)
+{
+    int rc = check_device_model(m);
+    if (rc) return rc;
+    if (iters_done) *iters_done = 0;
+    if (!re_in_dev || !out_re_dev || !out_im_dev || iters < 1 || !std::isfinite(tau) || !std::isfinite(t)) return HUBBARD_ERR_INVALID;
+    if (((uintptr_t)re_in_dev | (uintptr_t)im_in_dev | (uintptr_t)out_re_dev | (uintptr_t)out_im_dev) & 15) return HUBBARD_ERR_INVALID;
+    if (out_re_dev == out_im_dev) return HUBBARD_ERR_INVALID;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (m->dtype == HUBBARD_F32)
+        return lanczos_propagate_complex_impl<float>(m, static_cast<const float *>(re_in_dev), static_cast<const float *>(im_in_dev), iters,
+                                                     tau, t, static_cast<float *>(out_re_dev), static_cast<float *>(out_im_dev), iters_done, st);
+    return lanczos_propagate_complex_impl<double>(m, static_cast<const double *>(re_in_dev), static_cast<const double *>(im_in_dev), iters,
+                                                  tau, t, static_cast<double *>(out_re_dev), static_cast<double *>(out_im_dev), iters_done, st);
 }
 
 int hubbard_apply_host(hubbard_model *m, const void *x_host, void *y_host, void *stream)

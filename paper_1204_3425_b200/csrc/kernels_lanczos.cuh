@@ -154,4 +154,16 @@ vec_normalise_kernel(T *__restrict__ x, int64_t n, const LanczosScalars *S)
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) x[i] *= a;
 }
 
+// Complex propagation (lanczos_propagate_complex): A = sum_j Re(y_j) f_j and B = sum_j Im(y_j) f_j over the stacked
+// vectors f_j = [g_j ; h_j] (real part ; imaginary part); (y f) = (Re y g - Im y h) + i (Re y h + Im y g).
+template <typename T>
+__global__ void __launch_bounds__(kVecThreads)
+complex_mix_kernel(const T *__restrict__ A, const T *__restrict__ B, int64_t n, T *__restrict__ out_re, T *__restrict__ out_im)
+{
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        out_re[i] = A[i] - B[n + i];
+        if (out_im) out_im[i] = A[n + i] + B[i];
+    }
+}
+
 }  // namespace hub

@@ -127,6 +127,10 @@ struct hubbard_model {
     int coef_cap = 0;
     // staging for the *_host entry points
     void *stage[2] = {nullptr, nullptr};
+    // complex propagation: the same lattice with the up sector listed twice (real part ; imaginary part of a state
+    // stacked as one real vector), and three device buffers of 2 * dim elements
+    hubbard_model *twin = nullptr;
+    void *cplx[3] = {nullptr, nullptr, nullptr};
 
     bool profiling = false;
     std::vector<hub::ProfRecord> prof;

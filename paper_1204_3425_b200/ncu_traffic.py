@@ -1,8 +1,8 @@
 """Measurement bookkeeping for bench.py's `roofline.traffic` (no method arithmetic).
 
 `kernel_sources_hash()` identifies the kernel sources a DRAM-traffic figure was
-captured from; bench.py attaches a stored figure only while the hash still
-matches.  Run as a module to turn one `ncu --set full` capture into
+captured from (the gather sweeps of the headline path and the table layout they
+walk); bench.py attaches a stored figure only while the hash still matches.  Run as a module to turn one `ncu --set full` capture into
 profiles/ncu_traffic.json:
 
     ncu -i gpurun_out/prof.ncu-rep --page raw --csv > raw.csv
@@ -25,12 +25,15 @@ PKG = Path(__file__).resolve().parent
 OUT = PKG.parent / "profiles" / "ncu_traffic.json"
 
 
+# what decides the DRAM traffic of the captured kernels: the gather sweeps, their reductions, the table layout
+HASHED = ("kernels_gather.cuh", "kernels_common.cuh", "gather_tables.cpp", "gather_tables.h")
+
+
 def kernel_sources_hash() -> str:
     h = hashlib.sha256()
-    for p in sorted((PKG / "csrc").glob("*")):
-        if p.suffix in (".cu", ".cuh", ".h", ".cpp"):
-            h.update(p.name.encode())
-            h.update(p.read_bytes())
+    for name in HASHED:
+        h.update(name.encode())
+        h.update((PKG / "csrc" / name).read_bytes())
     return h.hexdigest()
 
 

@@ -650,6 +650,69 @@ def test_propagate_small_vs_dense_exponential(dtype, variant):
     assert np.max(np.abs(re2.double().cpu().numpy() - ref)) <= tol * np.max(np.abs(ref))
 
 
+@pytest.mark.parametrize("variant", ["paper", "twosweep", "gather", "persist", "auto"])
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_propagate_complex_small_vs_dense_exponential(dtype, variant):
+    """lanczos_propagate_complex (a second step of a time propagation: the state is complex) against
+    exp(-(tau + i t) H) psi from the dense eigen-decomposition of the definitional H (tier 0), complex psi; a real
+    psi (im = None) reproduces lanczos_propagate; in-place continuation; N_up != N_dn."""
+    for ns, nu, nd, bonds in ((6, 3, 3, ring_bonds(6)), (6, 2, 4, ladder_bonds(3, 2))):
+        tt, U = 1.0, 4.0
+        H = hd.dense_hamiltonian(ns, nu, nd, bonds, tt, U)
+        w, Q = np.linalg.eigh(H)
+        m = hb.hubbard_create(ns, nu, nd, bonds, tt, U, dtype)
+        m.hubbard_set_variant(VARIANTS[variant])
+        xr, _ = start_vector(31, m.dim, dtype)
+        xi, _ = start_vector(32, m.dim, dtype)
+        xr *= 1.3
+        xi *= 0.6
+        psi0 = xr.double().cpu().numpy() + 1j * xi.double().cpu().numpy()
+        tol = 1e-9 if dtype == "f64" else 2e-4
+        for tau, t in ((0.0, 0.35), (0.2, -0.15)):
+            ref = Q @ (np.exp(-(tau + 1j * t) * w) * (Q.T @ psi0))
+            re, im = torch.empty_like(xr), torch.empty_like(xr)
+            done = m.lanczos_propagate_complex(xr, xi, 60, tau, t, re, im)
+            assert done >= 1
+            got = re.double().cpu().numpy() + 1j * im.double().cpu().numpy()
+            assert np.max(np.abs(got - ref)) <= tol * np.max(np.abs(ref))
+            if tau == 0.0:
+                assert abs(np.linalg.norm(got) - np.linalg.norm(psi0)) <= tol * np.linalg.norm(psi0)
+        # real start vector: the same result as lanczos_propagate
+        re1, im1, re2, im2 = (torch.empty_like(xr) for _ in range(4))
+        m.lanczos_propagate(xr, 60, 0.0, 0.3, re1, im1)
+        m.lanczos_propagate_complex(xr, None, 60, 0.0, 0.3, re2, im2)
+        scale = float(xr.abs().max())
+        assert float((re1 - re2).abs().max()) <= tol * scale and float((im1 - im2).abs().max()) <= tol * scale
+        # two steps in place == one step of the summed time
+        a, b = xr.clone(), xi.clone()
+        m.lanczos_propagate_complex(a, b, 60, 0.0, 0.2, a, b)
+        m.lanczos_propagate_complex(a, b, 60, 0.0, 0.15, a, b)
+        ref = Q @ (np.exp(-1j * 0.35 * w) * (Q.T @ psi0))
+        got = a.double().cpu().numpy() + 1j * b.double().cpu().numpy()
+        assert np.max(np.abs(got - ref)) <= 2 * tol * np.max(np.abs(ref))
+
+
+def test_propagate_complex_C2_two_steps_vs_oracle_taylor():
+    """C2 at full size: two propagation steps (the second from a complex state) against the Taylor series of
+    exp(-i (t1 + t2) H) v evaluated with the ORACLE's matrix-free H; unitarity."""
+    c = CONFIGS["C2"]
+    m = hb.hubbard_create(c.n_sites, c.n_up, c.n_dn, c.bonds, c.t, 4.0, "f64")
+    ref = RefModel(c.n_sites, c.n_up, c.n_dn, c.bonds, c.t, 4.0)
+    v0, v0_np = start_vector(c.seed, c.dim, "f64")
+    re, im = torch.empty_like(v0), torch.empty_like(v0)
+    t1, t2 = 0.03, 0.02
+    m.lanczos_propagate(v0, 30, 0.0, t1, re, im)
+    m.lanczos_propagate_complex(re, im, 30, 0.0, t2, re, im)
+    psi = re.double().cpu().numpy() + 1j * im.double().cpu().numpy()
+    assert abs(np.linalg.norm(psi) - 1.0) <= 1e-10
+    t = t1 + t2
+    term, acc = v0_np.astype(complex), v0_np.astype(complex)
+    for k in range(1, 31):
+        term = (-1j * t / k) * (ref.apply(term.real) + 1j * ref.apply(term.imag))
+        acc = acc + term
+    assert np.max(np.abs(psi - acc)) <= 1e-10 * np.max(np.abs(acc))
+
+
 def test_propagate_C2_properties():
     """C2 at full size (no dense exponential): unitarity in real time and agreement with the Taylor series of
     exp(-i t H) v evaluated with the oracle's matrix-free H."""
