@@ -186,6 +186,25 @@ int lanczos_propagate(hubbard_model *m, const void *v0_dev, int iters, double ta
 int lanczos_propagate_complex(hubbard_model *m, const void *re_in_dev, const void *im_in_dev, int iters, double tau, double t,
                               void *out_re_dev, void *out_im_dev, int *iters_done, void *stream);
 
+/* ---- row-sharded H v and Lanczos pieces (several GPUs, one model per rank; "multi-GPU ... feasible") ----
+ * V is split by rows (up index): rank r owns rows [row0, row1).  The down term, the diagonal and the vector updates are
+ * local to the rows; the up term reads rows of every rank, so one H v needs the FULL x (the caller all-gathers the
+ * shards - the exchange step - and all-reduces the two scalars of an iteration).
+ *
+ * hubbard_apply_rows: y_rows = rows [row0, row1) of H x.  x_full_dev: all dim elements; y_rows_dev: (row1 - row0) *
+ * dim_dn elements, row a at (a - row0) * dim_dn; 16-byte aligned, not aliased.  Algorithms 2-4 per element (the
+ * kernel of variant PAPER restricted to the rows).  Enqueued on `stream`.
+ *
+ * lanczos_shard_update: one vector update of Algorithm 1 on a shard of n elements of the model's dtype, the scalar
+ * given by the caller, the shard's partial sum left in *result_dev (a device double, fixed summation order):
+ *   mode 0   inout = other - coef * inout   (line 4 with eq. 13: q = H f_j - b_j f_{j-1} over f_{j-1}),  *result = inout . f
+ *   mode 1   inout = inout - coef * f       (line 6),                                                    *result = |inout|^2
+ *   mode 2   inout = coef * inout           (line 11; other, f, result unused)
+ * Enqueued on `stream`; nothing is synchronised. */
+int hubbard_apply_rows(hubbard_model *m, const void *x_full_dev, void *y_rows_dev, int64_t row0, int64_t row1, void *stream);
+int lanczos_shard_update(hubbard_model *m, int mode, void *inout_dev, const void *other_dev, const void *f_dev, int64_t n,
+                         double coef, double *result_dev, void *stream);
+
 /* Breakdown threshold tau (>= 0; 0 = the paper's literal "b = 0" test). */
 int lanczos_set_tau(hubbard_model *m, double tau);
 

@@ -23,7 +23,7 @@ ABI_SYMBOLS = (
     "lanczos_ground_vector", "lanczos_propagate", "lanczos_propagate_complex", "lanczos_expm_e1", "lanczos_set_tau", "hubbard_apply_host",
     "lanczos_run_host", "hubbard_get_basis", "hubbard_get_hops", "hubbard_get_gather_table", "lanczos_ground_energy",
     "hubbard_profile", "hubbard_kernel_times", "hubbard_launch_count", "hubbard_last_cuda_error",
-    "hubbard_strerror", "hubbard_debug_set", "hubbard_debug_get",
+    "hubbard_strerror", "hubbard_debug_set", "hubbard_debug_get", "hubbard_apply_rows", "lanczos_shard_update",
 )
 
 
@@ -65,6 +65,8 @@ def _load() -> C.CDLL:
     lib.hubbard_launch_count.argtypes = [vp]
     lib.hubbard_launch_count.restype = i64
     lib.hubbard_last_cuda_error.argtypes = [vp]
+    lib.hubbard_apply_rows.argtypes = [vp, vp, vp, i64, i64, vp]
+    lib.lanczos_shard_update.argtypes = [vp, i32, vp, vp, vp, i64, dbl, vp, vp]
     lib.hubbard_debug_set.argtypes = [vp, C.c_char_p, i32]
     lib.hubbard_debug_get.argtypes = [vp, C.c_char_p, P(i32)]
     lib.hubbard_strerror.argtypes = [i32]
@@ -212,6 +214,18 @@ class Model:
                                              float(tau), float(t), _dptr(out_re), _dptr(out_im), C.byref(done), _stream(stream)),
                "lanczos_propagate_complex", self._h)
         return done.value
+
+    # -- row-sharded pieces (see sharded.py)
+    def hubbard_apply_rows(self, x_full, y_rows, row0, row1, stream=None):
+        _check(lib.hubbard_apply_rows(self._h, _dptr(x_full), _dptr(y_rows), int(row0), int(row1), _stream(stream)),
+               "hubbard_apply_rows", self._h)
+        return y_rows
+
+    def lanczos_shard_update(self, mode, inout, other, f, coef, result, stream=None):
+        _check(lib.lanczos_shard_update(self._h, int(mode), _dptr(inout), _dptr(other) if other is not None else None,
+                                        _dptr(f) if f is not None else None, inout.numel(), float(coef),
+                                        _dptr(result) if result is not None else None, _stream(stream)),
+               "lanczos_shard_update", self._h)
 
     # -- hot path, host buffers (numpy arrays or CPU torch tensors)
     @staticmethod

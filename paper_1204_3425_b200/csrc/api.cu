@@ -1073,6 +1073,7 @@ void hubbard_destroy(hubbard_model *m)
     for (int i = 0; i < 2; ++i) if (m->stage[i]) cudaFree(m->stage[i]);
     for (int i = 0; i < 3; ++i) if (m->cplx[i]) cudaFree(m->cplx[i]);
     if (m->twin) hubbard_destroy(m->twin);
+    if (m->shard_ticket) cudaFree(m->shard_ticket);
     if (m->d_scal) cudaFree(m->d_scal);
     if (m->d_partial) cudaFree(m->d_partial);
     if (m->d_alpha) cudaFree(m->d_alpha);
@@ -1202,6 +1203,59 @@ int lanczos_propagate_complex(hubbard_model *m, const void *re_in_dev, const voi
                                                      tau, t, static_cast<float *>(out_re_dev), static_cast<float *>(out_im_dev), iters_done, st);
     return lanczos_propagate_complex_impl<double>(m, static_cast<const double *>(re_in_dev), static_cast<const double *>(im_in_dev), iters,
                                                   tau, t, static_cast<double *>(out_re_dev), static_cast<double *>(out_im_dev), iters_done, st);
+}
+
+// ---- row-sharded H v and Lanczos pieces
+int hubbard_apply_rows(hubbard_model *m, const void *x_full_dev, void *y_rows_dev, int64_t row0, int64_t row1, void *stream)
+{
+    int rc = check_device_model(m);
+    if (rc) return rc;
+    if (!x_full_dev || !y_rows_dev || row0 < 0 || row1 < row0 || row1 > m->up.dim) return HUBBARD_ERR_INVALID;
+    if (((uintptr_t)x_full_dev | (uintptr_t)y_rows_dev) & 15) return HUBBARD_ERR_INVALID;
+    if (row1 == row0) return HUBBARD_OK;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    m->dev.U = m->U;
+    const DevModel &D = m->dev;
+    const int64_t bps = (D.dim_dn + kPaperThreads - 1) / kPaperThreads;
+    if (bps > 0x7fffffff) return HUBBARD_ERR_UNSUPPORTED;
+    const int64_t gy = std::min<int64_t>(row1 - row0, 65535);
+    auto launch = [&](auto tag) {
+        using T = decltype(tag);
+        SweepArgs<T> A{static_cast<const T *>(x_full_dev), static_cast<T *>(y_rows_dev), nullptr, m->d_partial};
+        A.a_begin = row0; A.a_end = row1;
+        ProfScope ps(m, 0, st);
+        hv_paper_kernel<T, false, 1><<<dim3((unsigned)bps, (unsigned)gy), kPaperThreads, (size_t)D.w_up * 4, st>>>(D, A);
+    };
+    if (m->dtype == HUBBARD_F32) launch(float{}); else launch(double{});
+    return after_launch(m);
+}
+
+int lanczos_shard_update(hubbard_model *m, int mode, void *inout_dev, const void *other_dev, const void *f_dev, int64_t n,
+                         double coef, double *result_dev, void *stream)
+{
+    int rc = check_device_model(m);
+    if (rc) return rc;
+    if (mode < 0 || mode > 2 || !inout_dev || n < 0 || !std::isfinite(coef)) return HUBBARD_ERR_INVALID;
+    if ((mode == 0 && (!other_dev || !f_dev)) || (mode == 1 && !f_dev) || (mode != 2 && !result_dev)) return HUBBARD_ERR_INVALID;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const int grid = lanczos_vec_grid(m, n);
+    if ((rc = ensure_partials(m, grid))) return rc;
+    if (!m->d_scal) CU_TRY(m, cudaMalloc((void **)&m->d_scal, sizeof(LanczosScalars)));
+    if (!m->shard_ticket) {
+        CU_TRY(m, cudaMalloc((void **)&m->shard_ticket, sizeof(unsigned)));
+        CU_TRY(m, cudaMemsetAsync(m->shard_ticket, 0, sizeof(unsigned), st));
+    }
+    auto launch = [&](auto tag) {
+        using T = decltype(tag);
+        T *io = static_cast<T *>(inout_dev);
+        const T *ot = static_cast<const T *>(other_dev), *ff = static_cast<const T *>(f_dev);
+        ProfScope ps(m, 3, st);
+        if (mode == 0) shard_update_kernel<T, 0><<<grid, kVecThreads, 0, st>>>(io, ot, ff, n, coef, m->d_partial, m->shard_ticket, result_dev);
+        else if (mode == 1) shard_update_kernel<T, 1><<<grid, kVecThreads, 0, st>>>(io, ot, ff, n, coef, m->d_partial, m->shard_ticket, result_dev);
+        else shard_update_kernel<T, 2><<<grid, kVecThreads, 0, st>>>(io, ot, ff, n, coef, m->d_partial, m->shard_ticket, result_dev);
+    };
+    if (m->dtype == HUBBARD_F32) launch(float{}); else launch(double{});
+    return after_launch(m);
 }
 
 int hubbard_apply_host(hubbard_model *m, const void *x_host, void *y_host, void *stream)

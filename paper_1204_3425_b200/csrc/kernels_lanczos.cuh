@@ -166,4 +166,42 @@ complex_mix_kernel(const T *__restrict__ A, const T *__restrict__ B, int64_t n, 
     }
 }
 
+// ---- row-sharded Lanczos: the vector updates of Algorithm 1 on ONE rank's shard of n elements.  The
+// scalars a_j, b_j come from the caller (all-reduced over the ranks); each kernel leaves its partial sum in
+// partials[0..gridDim.x) and the fixed-order total in *result (device), which the caller all-reduces.
+//   mode 0:  q = hf - b fprev   (lines 4 with eq. 13; written over fprev),  result = q . f      (line 5)
+//   mode 1:  w = q  - a f       (line 6; in place),                         result = w . w      (line 7)
+//   mode 2:  w = s w            (line 11)
+template <typename T, int MODE>
+__global__ void __launch_bounds__(kVecThreads)
+shard_update_kernel(T *__restrict__ inout, const T *__restrict__ other, const T *__restrict__ f, int64_t n, double coef,
+                    double *partials, unsigned *ticket, double *result)
+{
+    __shared__ double red[32];
+    __shared__ int flag;
+    const T cf = (T)coef;
+    double acc = 0.0;
+    const int64_t per = (n + gridDim.x - 1) / gridDim.x;
+    const int64_t lo = blockIdx.x * per, hi = min(n, lo + per);
+    for (int64_t i = lo + threadIdx.x; i < hi; i += blockDim.x) {
+        if (MODE == 0) {
+            const T q = other[i] - cf * inout[i];
+            inout[i] = q;
+            acc += (double)q * (double)f[i];
+        } else if (MODE == 1) {
+            const T w = inout[i] - cf * f[i];
+            inout[i] = w;
+            acc += (double)w * (double)w;
+        } else {
+            inout[i] = cf * inout[i];
+        }
+    }
+    if (MODE == 2) return;
+    const double s = block_sum(acc, red);
+    if (publish_and_check_last(s, partials, blockIdx.x, gridDim.x, ticket, &flag)) {
+        const double tot = sum_partials(partials, gridDim.x, red);
+        if (threadIdx.x == 0) { *result = tot; *ticket = 0; }
+    }
+}
+
 }  // namespace hub

@@ -19,6 +19,9 @@ struct SweepArgs {
     T *y;                  // u_prev in / q out (Lanczos), or y of hubbard_apply
     LanczosScalars *S;     // null for plain apply
     double *partials;
+    // row-sharded H v (hubbard_apply_rows): rows [a_begin, a_end) of the result from the FULL x; y holds only those
+    // rows (row a at (a - a_begin) * dim_dn).  a_end == 0 means all rows.
+    int64_t a_begin = 0, a_end = 0;
 };
 
 constexpr int kPaperThreads = 256;
@@ -52,10 +55,12 @@ hv_paper_kernel(DevModel M, SweepArgs<T> A)
     const int ndn = active ? M.dn_cnt[b] : 0;
     const uint32_t sdn = active ? M.st_dn[b] : 0u;
 
-    for (int64_t a0 = (int64_t)blockIdx.y * SUB; a0 < M.dim_up; a0 += (int64_t)gridDim.y * SUB) {
+    const int64_t a_end = A.a_end > 0 ? A.a_end : M.dim_up;
+    T *const yb = A.y - A.a_begin * M.dim_dn;            // row a of the result at yb + a * dim_dn
+    for (int64_t a0 = A.a_begin + (int64_t)blockIdx.y * SUB; a0 < a_end; a0 += (int64_t)gridDim.y * SUB) {
         int nup[SUB];
 #pragma unroll
-        for (int r = 0; r < SUB; ++r) nup[r] = (a0 + r < M.dim_up) ? M.up_cnt[a0 + r] : 0;
+        for (int r = 0; r < SUB; ++r) nup[r] = (a0 + r < a_end) ? M.up_cnt[a0 + r] : 0;
         __syncthreads();
 #pragma unroll
         for (int r = 0; r < SUB; ++r)
@@ -77,22 +82,22 @@ hv_paper_kernel(DevModel M, SweepArgs<T> A)
             uint32_t e = M.dn_ent32[(int64_t)k * M.ld_dn + b];
 #pragma unroll
             for (int r = 0; r < SUB; ++r)
-                if (a0 + r < M.dim_up) sum[r] += signed_by(e, A.x[(a0 + r) * M.dim_dn + (e >> 1)]);
+                if (a0 + r < a_end) sum[r] += signed_by(e, A.x[(a0 + r) * M.dim_dn + (e >> 1)]);
         }
 #pragma unroll
         for (int r = 0; r < SUB; ++r) {
             const int64_t a = a0 + r;
-            if (a >= M.dim_up) break;
+            if (a >= a_end) break;
             // Algorithm 4: on-the-fly diagonal
             const T xv = A.x[a * M.dim_dn + b];
             T h = tt * sum[r] + UU * (T)__popc(M.st_up[a] & sdn) * xv;
             if (LANCZOS) {
-                T *ya = A.y + a * M.dim_dn;
+                T *ya = yb + a * M.dim_dn;
                 T q = c_cur * h - bc * ya[b];
                 ya[b] = q;
                 acc += (double)q * (double)(c_cur * xv);
             } else {
-                A.y[a * M.dim_dn + b] = h;
+                yb[a * M.dim_dn + b] = h;
             }
         }
     }

@@ -129,6 +129,7 @@ struct hubbard_model {
     void *stage[2] = {nullptr, nullptr};
     // complex propagation: the same lattice with the up sector listed twice (real part ; imaginary part of a state
     // stacked as one real vector), and three device buffers of 2 * dim elements
+    unsigned *shard_ticket = nullptr;   // arrival counter of the row-sharded vector kernels
     hubbard_model *twin = nullptr;
     void *cplx[3] = {nullptr, nullptr, nullptr};
 

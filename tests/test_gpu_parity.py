@@ -761,3 +761,100 @@ def test_cluster_row_sweep(name, ns, nu, nd, bonds, R, NC, dtype):
     a_ref, b_ref = lr.lanczos(ref.apply, x_np, 40)
     e_ref = lr.ground_energy(a_ref, b_ref)
     assert abs(hb.lanczos_ground_energy(alpha, beta) - e_ref) <= TOL_E0[dtype] * abs(e_ref)
+
+
+# ---------------------------------------------------------------- SURVEY 8(f)-3
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("name,ns,nu,nd,bonds", [("C2", 12, 6, 6, ring_bonds(12)), ("odd", 7, 3, 4, ring_bonds(7) + [(0, 3), (2, 6)])])
+def test_sharded_apply_rows(name, ns, nu, nd, bonds, dtype):
+    """hubbard_apply_rows: the rows of H x for arbitrary row ranges (unequal shards, a single row, the empty range)
+    assemble to the oracle's H x."""
+    from paper_1204_3425_b200 import sharded
+    ref = RefModel(ns, nu, nd, bonds, 1.0, 4.0)
+    m = hb.hubbard_create(ns, nu, nd, bonds, 1.0, 4.0, dtype)
+    x, x_np = start_vector(123, m.dim, dtype)
+    y_ref = ref.apply(x_np)
+    for world in (1, 3, 8):
+        y = torch.full_like(x, float("nan"))
+        for r0, r1 in sharded.row_partition(m.dim_up, world):
+            yr = torch.full(((r1 - r0) * m.dim_dn,), float("nan"), dtype=x.dtype, device=x.device)
+            m.hubbard_apply_rows(x, yr, r0, r1)
+            y[r0 * m.dim_dn:r1 * m.dim_dn] = yr
+        torch.cuda.synchronize()
+        assert rel_max_err(y, y_ref) <= TOL_HV[dtype]
+    with pytest.raises(hb.HubbardError):
+        m.hubbard_apply_rows(x, y, 2, m.dim_up + 1)
+
+
+def _run_virtual_ranks(m, world, v0, iters, tau):
+    """Drives `world` instances of sharded_lanczos in lock-step on one GPU: each exchange step is resolved when every
+    rank has reached it (threads + barriers; the kernels of different ranks simply queue on the stream)."""
+    import threading
+    from paper_1204_3425_b200 import sharded
+    parts = sharded.row_partition(m.dim_up, world)
+    bar = threading.Barrier(world)
+    slots = {"gather": [None] * world, "reduce": [None] * world}
+    results = [None] * world
+
+    class Coll:
+        def __init__(self, rank):
+            self.rank = rank
+
+        def all_gather_rows(self, shard, parts_, dim_dn, out_full):
+            slots["gather"][self.rank] = shard
+            bar.wait()
+            for r, (r0, r1) in enumerate(parts_):
+                out_full[r0 * dim_dn:r1 * dim_dn].copy_(slots["gather"][r])
+            torch.cuda.synchronize()
+            bar.wait()
+            return out_full
+
+        def all_reduce_sum(self, scalar):
+            slots["reduce"][self.rank] = float(scalar.item())
+            bar.wait()
+            tot = sum(slots["reduce"])            # same order on every rank
+            bar.wait()
+            return tot
+
+    def work(rank):
+        torch.cuda.set_device(0)
+        r0, r1 = parts[rank]
+        ops = sharded.LibraryOps(models[rank], dev())
+        results[rank] = sharded.sharded_lanczos(ops, Coll(rank), rank, world, m.dim_up, m.dim_dn,
+                                                v0[r0 * m.dim_dn:r1 * m.dim_dn].clone(), iters, tau)
+
+    models = [m] + [None] * (world - 1)
+    return models, work, results
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_sharded_lanczos_virtual_ranks_vs_oracle(dtype):
+    """The row-sharded Lanczos with the LIBRARY's kernels behind it (hubbard_apply_rows, lanczos_shard_update), three
+    ranks' shards driven in lock-step on one GPU, against Algorithm 1 on the oracle: coefficient prefix, E_0, and the
+    same numbers on every rank.  (The multi-process exchange itself is covered on CPU: tests/test_sharded_cpu.py.)"""
+    import threading
+    c = CONFIGS["C2"]
+    world, iters = 3, 60
+    ref = RefModel(c.n_sites, c.n_up, c.n_dn, c.bonds, c.t, 4.0)
+    v0, v0_np = start_vector(c.seed, c.dim, dtype)
+    m0 = hb.hubbard_create(c.n_sites, c.n_up, c.n_dn, c.bonds, c.t, 4.0, dtype)
+    models, work, results = _run_virtual_ranks(m0, world, v0, iters, 1e-10 if dtype == "f64" else 1e-5)
+    for r in range(1, world):                     # one model per rank, as on several GPUs
+        models[r] = hb.hubbard_create(c.n_sites, c.n_up, c.n_dn, c.bonds, c.t, 4.0, dtype)
+    threads = [threading.Thread(target=work, args=(r,)) for r in range(world)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join(timeout=600)
+    assert all(r is not None for r in results)
+    a_ref, b_ref = lr.lanczos(ref.apply, v0_np, iters)
+    n = 30
+    tol_c = 1e-10 if dtype == "f64" else 1e-5
+    for alpha, beta in results:
+        alpha, beta = np.array(alpha), np.array(beta)
+        assert len(alpha) == iters
+        assert np.max(np.abs(alpha[:n] - a_ref[:n]) / np.maximum(1.0, np.abs(a_ref[:n]))) <= tol_c
+        assert np.max(np.abs(beta[:n] - b_ref[:n]) / np.maximum(1.0, np.abs(b_ref[:n]))) <= tol_c
+        e_ref = lr.ground_energy(a_ref, b_ref)
+        assert abs(hb.lanczos_ground_energy(alpha, beta) - e_ref) <= TOL_E0[dtype] * abs(e_ref)
+    assert results[0] == results[1] == results[2]
