@@ -58,6 +58,9 @@ constexpr int kGatherBatch = kSlotBatch; // hop entries per batch (gather_tables
 #ifndef GS_L2PF
 #define GS_L2PF 1
 #endif
+#ifndef GS_TMA_STAGE
+#define GS_TMA_STAGE 1    // COL sweep: stage the tile with cp.async.bulk + mbarrier instead of per-thread loads
+#endif
 #ifndef GS_STAGE_UNROLL
 #define GS_STAGE_UNROLL 1
 #endif
@@ -165,6 +168,37 @@ __device__ __forceinline__ void lanczos_rotate(LanczosScalars *S, double b2, dou
     }
     S->started += 1;
     S->ticket = 0;
+}
+
+// ------------------------------------------------------------------ bulk (TMA) staging of a contiguous tile
+// cp.async.bulk moves a contiguous block global -> shared memory without occupying threads, registers or the
+// LSU; completion is counted in bytes on an mbarrier in shared memory.
+__device__ __forceinline__ uint32_t smem_addr_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_addr_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_addr_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_addr_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *dst_smem, const void *src_gmem, unsigned bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_addr_u32(dst_smem)),
+                 "l"(src_gmem), "r"(bytes), "r"(smem_addr_u32(bar))
+                 : "memory");
 }
 
 // ------------------------------------------------------------------ helpers
@@ -353,6 +387,7 @@ gather_sweep_kernel(GatherArgs<T> A)
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ double red[32];
     __shared__ int flag;
+    __shared__ __align__(8) uint64_t stage_bar;           // COL: bytes of the bulk-staged tile that have landed
     using PR = Pack<T, R>;
     using EB = Pack<E, kGatherBatch>;
     PR *Xs = reinterpret_cast<PR *>(smem_raw);            // [n_in_p + kZeroSlots]
@@ -396,6 +431,13 @@ gather_sweep_kernel(GatherArgs<T> A)
     for (int i = threadIdx.x; i < n_in_w / 32; i += nthr) wsl_s[i] = A.in.wslots[i];   // slots per warp of positions
     double racc = 0.0;                                    // |w|^2 (ROW) or q.f (COL) partial
     const int64_t tile_bytes = (int64_t)n_in_p * (int64_t)sizeof(PR);
+    // COL stages one contiguous block with no arithmetic on the way: a bulk copy when it is 16-byte granular
+    const bool bulk_stage = COL && GS_TMA_STAGE && (tile_bytes % 16) == 0;
+    unsigned stage_parity = 0;
+    if (bulk_stage && threadIdx.x == 0) {
+        mbar_init(&stage_bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
     const int n_it = (n_in_w + nthr - 1) / nthr;                // gather iterations per tile
     // Position handled by this thread in iteration `it`: stripes of nthr positions, the warps of every other
     // stripe mirrored, so that with positions ordered by descending hop count all warps get equal work.
@@ -445,6 +487,18 @@ gather_sweep_kernel(GatherArgs<T> A)
                         }
                     }
                 }
+            } else if (bulk_stage) {
+                // (the barrier above ordered the previous tile's shared-memory reads; the proxy fence orders them
+                // against the asynchronous writes that follow)
+                if (threadIdx.x == 0) {
+                    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                    mbar_expect_tx(&stage_bar, (unsigned)tile_bytes);
+                    constexpr int64_t kChunk = 32768;
+                    for (int64_t off = 0; off < tile_bytes; off += kChunk)
+                        bulk_g2s(smem_raw + off, reinterpret_cast<const char *>(src) + off, (unsigned)min(kChunk, tile_bytes - off), &stage_bar);
+                }
+                mbar_wait(&stage_bar, stage_parity);
+                stage_parity ^= 1u;
             } else {
                 for (int i0 = threadIdx.x; i0 < n_in_p; i0 += kStageUnroll * nthr) {
                     PR v[kStageUnroll];
