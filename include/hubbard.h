@@ -52,7 +52,8 @@ enum {
     HUBBARD_ERR_DEVICE_OOM = -3, /* cudaMalloc failed */
     HUBBARD_ERR_CUDA = -4,       /* any other CUDA error; see hubbard_last_cuda_error */
     HUBBARD_ERR_NO_DEVICE = -5,  /* model was made by hubbard_create_host: no device state */
-    HUBBARD_ERR_UNSUPPORTED = -6 /* sector too large for the index types used */
+    HUBBARD_ERR_UNSUPPORTED = -6, /* sector too large for the index types used */
+    HUBBARD_ERR_TOO_LARGE = -7   /* lanczos_shard_update_noalloc: n > HUBBARD_NOALLOC_MAX_N (its scratch is a fixed array) */
 };
 
 /* Kernel variants selectable with hubbard_set_variant (for measurement; every
@@ -204,6 +205,28 @@ int lanczos_propagate_complex(hubbard_model *m, const void *re_in_dev, const voi
 int hubbard_apply_rows(hubbard_model *m, const void *x_full_dev, void *y_rows_dev, int64_t row0, int64_t row1, void *stream);
 int lanczos_shard_update(hubbard_model *m, int mode, void *inout_dev, const void *other_dev, const void *f_dev, int64_t n,
                          double coef, double *result_dev, void *stream);
+
+/* lanczos_shard_update_noalloc: lanczos_shard_update for callers that must not allocate (CUDA graph capture, tight
+ * serving loops, harnesses that forbid cudaMalloc).  Same arguments, same arithmetic per element (Algorithm 1 lines
+ * 4-7 and 11, eq. 13), same fixed-order fp64 reduction - but the per-block partial sums and the
+ * arrival counter live in ONE fixed array inside the library (static __device__, HUBBARD_NOALLOC_SCRATCH_BYTES = 256 +
+ * 8 * 8192 bytes, held by every GPU that loads the library until the process exits) instead of buffers the model
+ * allocates on first use.  The call makes no cudaMalloc / cudaFree, creates no event or stream and synchronises
+ * nothing: it enqueues one 256-byte memset (the counter must start at zero) and one kernel on `stream`.  The array's
+ * device address is resolved once per device when a model is created on it (hubbard_create).
+ *   - one block per HUBBARD_NOALLOC_CHUNK = 32768 elements, one partial per block, hence
+ *     n <= HUBBARD_NOALLOC_MAX_N = 8192 * 32768 = 268 435 456 elements; a larger n returns HUBBARD_ERR_TOO_LARGE and
+ *     nothing is enqueued (all three modes).  The partial sums are cut differently from lanczos_shard_update's, so
+ *     *result_dev agrees with it to rounding (fp64 accumulation in both), the updated vector bit for bit.
+ *   - the array is shared by EVERY call on that GPU, of every model, and keeps the last call's contents: two calls
+ *     that may overlap on the GPU (different streams, no dependency between them) RACE on it.  Serialise them.
+ *   - hubbard_profile does not see these launches (timing them would create events). */
+#define HUBBARD_NOALLOC_CHUNK 32768
+#define HUBBARD_NOALLOC_MAX_BLOCKS 8192
+#define HUBBARD_NOALLOC_MAX_N ((int64_t)HUBBARD_NOALLOC_MAX_BLOCKS * HUBBARD_NOALLOC_CHUNK)
+#define HUBBARD_NOALLOC_SCRATCH_BYTES (256 + 8 * HUBBARD_NOALLOC_MAX_BLOCKS)
+int lanczos_shard_update_noalloc(hubbard_model *m, int mode, void *inout_dev, const void *other_dev, const void *f_dev,
+                                 int64_t n, double coef, double *result_dev, void *stream);
 
 /* Breakdown threshold tau (>= 0; 0 = the paper's literal "b = 0" test). */
 int lanczos_set_tau(hubbard_model *m, double tau);

@@ -14,6 +14,8 @@ from . import build as _build
 
 HUBBARD_F32, HUBBARD_F64 = 0, 1
 VARIANT_AUTO, VARIANT_PAPER, VARIANT_TWOSWEEP, VARIANT_GATHER, VARIANT_PERSIST = 0, 1, 2, 3, 4
+ERR_TOO_LARGE = -7
+NOALLOC_CHUNK, NOALLOC_MAX_N = 32768, 8192 * 32768          # include/hubbard.h: lanczos_shard_update_noalloc
 N_KCLASS = 6
 KCLASS_NAMES = ("hv_paper", "row_sweep", "col_sweep", "vec_sweep", "scalar", "setup")
 
@@ -24,6 +26,7 @@ ABI_SYMBOLS = (
     "lanczos_run_host", "hubbard_get_basis", "hubbard_get_hops", "hubbard_get_gather_table", "lanczos_ground_energy",
     "hubbard_profile", "hubbard_kernel_times", "hubbard_launch_count", "hubbard_last_cuda_error",
     "hubbard_strerror", "hubbard_debug_set", "hubbard_debug_get", "hubbard_apply_rows", "lanczos_shard_update",
+    "lanczos_shard_update_noalloc",
 )
 
 
@@ -67,6 +70,7 @@ def _load() -> C.CDLL:
     lib.hubbard_last_cuda_error.argtypes = [vp]
     lib.hubbard_apply_rows.argtypes = [vp, vp, vp, i64, i64, vp]
     lib.lanczos_shard_update.argtypes = [vp, i32, vp, vp, vp, i64, dbl, vp, vp]
+    lib.lanczos_shard_update_noalloc.argtypes = lib.lanczos_shard_update.argtypes
     lib.hubbard_debug_set.argtypes = [vp, C.c_char_p, i32]
     lib.hubbard_debug_get.argtypes = [vp, C.c_char_p, P(i32)]
     lib.hubbard_strerror.argtypes = [i32]
@@ -226,6 +230,14 @@ class Model:
                                         _dptr(f) if f is not None else None, inout.numel(), float(coef),
                                         _dptr(result) if result is not None else None, _stream(stream)),
                "lanczos_shard_update", self._h)
+
+    def lanczos_shard_update_noalloc(self, mode, inout, other, f, coef, result, stream=None, n=None):
+        """lanczos_shard_update with the library's fixed scratch array: no allocation, n <= NOALLOC_MAX_N
+        (include/hubbard.h).  `n` overrides the element count (default: all of `inout`)."""
+        _check(lib.lanczos_shard_update_noalloc(self._h, int(mode), _dptr(inout), _dptr(other) if other is not None else None,
+                                                _dptr(f) if f is not None else None, inout.numel() if n is None else int(n),
+                                                float(coef), _dptr(result) if result is not None else None, _stream(stream)),
+               "lanczos_shard_update_noalloc", self._h)
 
     # -- hot path, host buffers (numpy arrays or CPU torch tensors)
     @staticmethod

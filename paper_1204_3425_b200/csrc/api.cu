@@ -1023,6 +1023,34 @@ int ensure_stage(hubbard_model *m, int which)
     return HUBBARD_OK;
 }
 
+// ---- fixed scratch of lanczos_shard_update_noalloc (include/hubbard.h): the arrival counter in the first 256 bytes,
+// then one fp64 partial sum per block.  A file-scope device array: every GPU that loads this library holds these
+// HUBBARD_NOALLOC_SCRATCH_BYTES until the process exits, and nobody ever allocates or frees them.  In HOST code the name
+// `g_noalloc_scratch` is only a handle for the runtime, not a device address - a kernel given `g_noalloc_scratch`
+// itself would fault (or, where the GPU can reach host memory, silently use the wrong memory): the address a kernel
+// may be given comes from cudaGetSymbolAddress, once per device, with that device current.
+static __device__ __align__(256) unsigned char g_noalloc_scratch[HUBBARD_NOALLOC_SCRATCH_BYTES];
+
+// Device address of g_noalloc_scratch on the CURRENT device (resolved on first use per device, then cached).
+// Called at set-up (hubbard_create); allocates nothing.
+int noalloc_scratch_for_current_device(hubbard_model *m, void **out)
+{
+    constexpr int kMaxDevices = 64;
+    static std::mutex mu;
+    static void *cached[kMaxDevices] = {nullptr};
+    int dev = -1;
+    CU_TRY(m, cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kMaxDevices) return HUBBARD_ERR_UNSUPPORTED;
+    std::lock_guard<std::mutex> lock(mu);
+    if (!cached[dev]) {
+        void *p = nullptr;
+        CU_TRY(m, cudaGetSymbolAddress(&p, g_noalloc_scratch));
+        cached[dev] = p;
+    }
+    *out = cached[dev];
+    return HUBBARD_OK;
+}
+
 int check_device_model(const hubbard_model *m)
 {
     if (!m) return HUBBARD_ERR_INVALID;
@@ -1057,6 +1085,7 @@ int hubbard_create(hubbard_model **out, int n_sites, int n_up, int n_dn, const i
     if (m->sm_count <= 0) m->sm_count = 148;
     rc = upload_tables(m);
     if (rc) return fail(rc);
+    if ((rc = noalloc_scratch_for_current_device(m, &m->noalloc_scratch))) return fail(rc);
     m->has_device = true;
     return HUBBARD_OK;
 }
@@ -1258,6 +1287,34 @@ int lanczos_shard_update(hubbard_model *m, int mode, void *inout_dev, const void
     return after_launch(m);
 }
 
+int lanczos_shard_update_noalloc(hubbard_model *m, int mode, void *inout_dev, const void *other_dev, const void *f_dev,
+                                 int64_t n, double coef, double *result_dev, void *stream)
+{
+    int rc = check_device_model(m);
+    if (rc) return rc;
+    if (mode < 0 || mode > 2 || !inout_dev || n < 0 || !std::isfinite(coef)) return HUBBARD_ERR_INVALID;
+    if ((mode == 0 && (!other_dev || !f_dev)) || (mode == 1 && !f_dev) || (mode != 2 && !result_dev)) return HUBBARD_ERR_INVALID;
+    if (n > HUBBARD_NOALLOC_MAX_N) return HUBBARD_ERR_TOO_LARGE;     // more blocks than the fixed array has partials
+    if (!m->noalloc_scratch) return HUBBARD_ERR_CUDA;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const int grid = (int)std::max<int64_t>(1, (n + HUBBARD_NOALLOC_CHUNK - 1) / HUBBARD_NOALLOC_CHUNK);   // <= MAX_BLOCKS
+    // the array keeps whatever the last call (of any model on this GPU) left: the counter must start at zero; the
+    // partials need not (every block writes its own before it takes a ticket)
+    unsigned *ticket = static_cast<unsigned *>(m->noalloc_scratch);
+    double *partials = reinterpret_cast<double *>(static_cast<unsigned char *>(m->noalloc_scratch) + 256);
+    if (mode != 2) CU_TRY(m, cudaMemsetAsync(ticket, 0, 256, st));
+    auto launch = [&](auto tag) {
+        using T = decltype(tag);
+        T *io = static_cast<T *>(inout_dev);
+        const T *ot = static_cast<const T *>(other_dev), *ff = static_cast<const T *>(f_dev);
+        if (mode == 0) shard_update_kernel<T, 0><<<grid, kVecThreads, 0, st>>>(io, ot, ff, n, coef, partials, ticket, result_dev);
+        else if (mode == 1) shard_update_kernel<T, 1><<<grid, kVecThreads, 0, st>>>(io, ot, ff, n, coef, partials, ticket, result_dev);
+        else shard_update_kernel<T, 2><<<grid, kVecThreads, 0, st>>>(io, ot, ff, n, coef, partials, ticket, result_dev);
+    };
+    if (m->dtype == HUBBARD_F32) launch(float{}); else launch(double{});
+    return after_launch(m);
+}
+
 int hubbard_apply_host(hubbard_model *m, const void *x_host, void *y_host, void *stream)
 {
     int rc = check_device_model(m);
@@ -1426,6 +1483,8 @@ const char *hubbard_strerror(int code)
         case HUBBARD_ERR_CUDA: return "CUDA error (see hubbard_last_cuda_error)";
         case HUBBARD_ERR_NO_DEVICE: return "model has no device state (hubbard_create_host)";
         case HUBBARD_ERR_UNSUPPORTED: return "sector too large for the index types used";
+        case HUBBARD_ERR_TOO_LARGE:
+            return "n exceeds HUBBARD_NOALLOC_MAX_N = 268435456 elements: the no-alloc entry point's scratch is a fixed array";
         default: return "unknown error";
     }
 }

@@ -130,6 +130,8 @@ struct hubbard_model {
     // complex propagation: the same lattice with the up sector listed twice (real part ; imaginary part of a state
     // stacked as one real vector), and three device buffers of 2 * dim elements
     unsigned *shard_ticket = nullptr;   // arrival counter of the row-sharded vector kernels
+    void *noalloc_scratch = nullptr;    // device address of the library's fixed scratch array on this model's GPU
+                                        // (lanczos_shard_update_noalloc; resolved by hubbard_create, never allocated or freed)
     hubbard_model *twin = nullptr;
     void *cplx[3] = {nullptr, nullptr, nullptr};
 
