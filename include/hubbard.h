@@ -318,6 +318,9 @@ int64_t hubbard_launch_count(const hubbard_model *m);
  *   "gather_nosort" (0/1)     the Lanczos work vectors of variant GATHER keep the basis order
  *   "gather_nosymmetry" (0/1) their internal order comes from hop counts only (no lattice-symmetry orbits)
  *   "gather_ctas" (1-4)       CTAs per SM for small tiles
+ *   "gather_fold" (0/1)       1 (default): lanczos_* of variant GATHER in the folded, eight-pass form (the ROW sweep parks
+ *                             its tile of u_j in tensor memory and applies "- b_{j+1} f_j" of Algorithm 1 line 4 itself);
+ *                             0: the nine-pass form (the COL sweep reads u_j).  DESIGN.md 2 (readings) and 4.2
  *   "apply_pure_gather" (0/1) plain hubbard_apply as two gather sweeps instead of the hybrid
  *   "twosweep_old_row" (0/1)  AUTO's TWOSWEEP fallback keeps the first row kernel
  *   "row_R" (0-4), "strip_mb" (1-1024), "strip_rb"   geometry of variant TWOSWEEP (0 = automatic)
@@ -328,7 +331,8 @@ int64_t hubbard_launch_count(const hubbard_model *m);
  *                             take / avoid the cluster row sweep of rows larger than one SM, force one (R, NC)
  * Options that change a device table layout re-upload that table (host work + cudaMemcpy; no kernel launch).
  * hubbard_debug_get returns an option, or what the library resolved for this model: "resolved_variant"
- * (HUBBARD_VARIANT_* that AUTO stands for), "resolved_gather_R", "resolved_gather_symmetry" (order of the lattice symmetry group the
+ * (HUBBARD_VARIANT_* that AUTO stands for), "resolved_gather_R", "resolved_gather_fold" (tensor-memory columns one
+ * CTA of the folded ROW sweep allocates, 0 = nine-pass form), "resolved_gather_symmetry" (order of the lattice symmetry group the
  * internal order of variant GATHER was built from, 0 = none), "resolved_cluster_row", "resolved_cluster_R",
  * "resolved_cluster_NC".  Unknown key or out-of-range value: HUBBARD_ERR_INVALID. */
 int hubbard_debug_set(hubbard_model *m, const char *key, int value);

@@ -335,6 +335,35 @@ size_t gather_smem_bytes(int64_t n_in_p, int R, size_t es)
     return (size_t)(n_in_p + 128 / (R * es)) * R * es + (size_t)(round_up(n_in_p, 32) / 32) * sizeof(uint16_t);
 }
 
+// Small sectors: several CTAs per SM (their staging and gather phases overlap one another); the 64-register
+// kernels allow 1024 threads per SM in total.
+void gather_launch_shape(const hubbard_model *m, size_t smem, int *per_sm, int *threads)
+{
+    int n = (int)std::min<size_t>(4, (size_t)(m->max_smem_optin - 2048) / (smem + 1024));
+    n = std::max(1, std::min(n, m->opt.gather_ctas));
+    *per_sm = n;
+    *threads = std::max(32, kGatherMaxThreads / n / 32 * 32);
+}
+
+// Folded Lanczos form of variant GATHER: tensor-memory columns one CTA of the ROW sweep needs to park its tile of u_j
+// (one 16-byte piece per thread and gather iteration; a warp addresses a quarter of the 128 lanes), as the power of
+// two >= 32 that tcgen05.alloc takes.  0: the nine-pass form (knob off, or the resident CTAs of an SM would need more
+// than its 512 columns).
+int gather_fold_cols(const hubbard_model *m)
+{
+    const int R = gather_R(m);
+    if (!m->opt.gather_fold || R == 0) return 0;
+    const size_t es = m->dtype == HUBBARD_F32 ? 4 : 8;
+    const int64_t dd_p = round_up(m->dn.dim, gather_align(m));
+    int per_sm, threads;
+    gather_launch_shape(m, gather_smem_bytes(dd_p, R, es), &per_sm, &threads);
+    const int64_t n_it = (round_up(dd_p, 32) + threads - 1) / threads;
+    const int64_t need = (int64_t)((threads / 32 + 3) / 4) * n_it * (int64_t)(R * es / 4);
+    int64_t cols = 32;
+    while (cols < need) cols *= 2;
+    return (cols * per_sm <= 512) ? (int)cols : 0;
+}
+
 template <typename T, int R, typename E, bool COL, bool LZ>
 int launch_gather_inst(hubbard_model *m, GatherArgs<T> A, cudaStream_t st)
 {
@@ -345,11 +374,8 @@ int launch_gather_inst(hubbard_model *m, GatherArgs<T> A, cudaStream_t st)
     const size_t smem = gather_smem_bytes(n_in_p, R, sizeof(T));
     if (int rc = ensure_smem(m, kern, smem, true)) return rc;
     const int64_t tiles = (COL ? A.dd_p : A.du_p) / R;
-    // Small sectors: several CTAs per SM (their staging and gather phases overlap one another); the 64-register
-    // kernels allow 1024 threads per SM in total.
-    int per_sm = (int)std::min<size_t>(4, (size_t)(m->max_smem_optin - 2048) / (smem + 1024));
-    per_sm = std::max(1, std::min(per_sm, m->opt.gather_ctas));
-    const int threads = std::max(32, kGatherMaxThreads / per_sm / 32 * 32);
+    int per_sm, threads;
+    gather_launch_shape(m, smem, &per_sm, &threads);
     const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(tiles, (int64_t)m->sm_count * per_sm));
     {
         ProfScope ps(m, COL ? 2 : 1, st);
@@ -368,7 +394,12 @@ int launch_gather(hubbard_model *m, GatherArgs<T> A, cudaStream_t st)
     A.dim_up = D.dim_up; A.dim_dn = D.dim_dn; A.t = m->t; A.U = m->U;
     const int R = gather_R(m);
     if (R == 0) return HUBBARD_ERR_INVALID;
-    if (LZ) { int rc = ensure_partials(m, (int64_t)m->sm_count * 4); if (rc) return rc; A.partials = m->d_partial; }
+    if (LZ) {
+        // (two partials per block: q.f and |q|^2 of the COL sweep)
+        int rc = ensure_partials(m, (int64_t)m->sm_count * 8); if (rc) return rc;
+        A.partials = m->d_partial;
+        A.fold_cols = gather_fold_cols(m);
+    }
     if (!A.in.e16) {
         if constexpr (sizeof(T) == 4) {
             if (R == 1) return launch_gather_inst<T, 1, uint32_t, COL, LZ>(m, A, st);
@@ -679,7 +710,7 @@ int lanczos_gather_steps(hubbard_model *m, const T *v0, const LanczosPlan &P, cu
     int rc;
     const int64_t n_p = gather_vec_elems(m);
     const int vec_grid = lanczos_vec_grid(m, n_p);
-    if ((rc = ensure_partials(m, std::max<int64_t>(vec_grid, (int64_t)m->sm_count * 4)))) return rc;
+    if ((rc = ensure_partials(m, std::max<int64_t>(vec_grid, (int64_t)m->sm_count * 8)))) return rc;
     T *rt[2] = {static_cast<T *>(m->work[0]), static_cast<T *>(m->work[1])};
     T *wct[2] = {static_cast<T *>(m->work[2]), static_cast<T *>(m->work[3])};
     T *zct = static_cast<T *>(m->work[4]);
@@ -1396,6 +1427,7 @@ const OptKey kOptKeys[] = {
     {"gather_nosort", &hub::DebugOptions::gather_nosort, true, 0, 1},
     {"gather_nosymmetry", &hub::DebugOptions::gather_nosymmetry, true, 0, 1},
     {"gather_ctas", &hub::DebugOptions::gather_ctas, false, 1, 4},
+    {"gather_fold", &hub::DebugOptions::gather_fold, false, 0, 1},
     {"apply_pure_gather", &hub::DebugOptions::apply_pure_gather, false, 0, 1},
     {"twosweep_old_row", &hub::DebugOptions::twosweep_old_row, false, 0, 1},
     {"row_R", &hub::DebugOptions::row_R, false, 0, 4},
@@ -1436,6 +1468,7 @@ int hubbard_debug_get(const hubbard_model *m, const char *key, int *value)
     // what the library resolved (read-only)
     if (!std::strcmp(key, "resolved_variant")) { *value = m->has_device ? resolve_variant(m) : m->variant; return HUBBARD_OK; }
     if (!std::strcmp(key, "resolved_gather_R")) { *value = m->gather_R; return HUBBARD_OK; }
+    if (!std::strcmp(key, "resolved_gather_fold")) { *value = m->has_device ? gather_fold_cols(m) : 0; return HUBBARD_OK; }
     if (!std::strcmp(key, "resolved_gather_symmetry")) { *value = m->gather_symmetry; return HUBBARD_OK; }
     if (!std::strcmp(key, "resolved_cluster_row")) { *value = m->cluster_row; return HUBBARD_OK; }
     if (!std::strcmp(key, "resolved_cluster_R")) { *value = m->cluster_R; return HUBBARD_OK; }

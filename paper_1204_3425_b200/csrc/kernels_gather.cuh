@@ -61,6 +61,9 @@ constexpr int kGatherBatch = kSlotBatch; // hop entries per batch (gather_tables
 #ifndef GS_TMA_STAGE
 #define GS_TMA_STAGE 1    // COL sweep: stage the tile with cp.async.bulk + mbarrier instead of per-thread loads
 #endif
+#ifndef GS_FOLD_LATE
+#define GS_FOLD_LATE 1    // folded ROW sweep: take the parked piece back after the gather (1.96 ms) instead of before it (1.98 ms)
+#endif
 #ifndef GS_STAGE_UNROLL
 #define GS_STAGE_UNROLL 1
 #endif
@@ -84,6 +87,9 @@ struct GatherArgs {
     double *partials;
     double *alpha_out, *beta_out;
     int y_rowmajor;         // ROW sweep of hubbard_apply writes y row-major (no CT buffers): hybrid with the strip sweep
+    // Lanczos, folded (eight-pass) form: tensor-memory columns the ROW sweep allocates to park u_j (0: nine-pass form,
+    // the COL sweep reads u_j in CT)
+    int fold_cols;
 };
 
 template <typename T, int N>
@@ -377,6 +383,65 @@ __device__ __forceinline__ void hop_batch_n(const unsigned char *xs_bytes, const
     }
 }
 
+// ------------------------------------------------------------------ tensor memory as a per-thread parking buffer
+// Folded Lanczos form (ROW sweep): the tile fills the shared memory, and the epilogue of a position needs the piece of
+// u_j that the same thread loaded while staging it.  The SM's 256 KB of tensor memory (128 lanes x 512 columns x 4
+// bytes, otherwise unused by this library) holds it: warp w owns lanes 32 (w % 4) .. + 31 (the only ones it can
+// address), a thread parks its piece with tcgen05.st (SASS STTM) and takes the same piece back with tcgen05.ld
+// (LDTM) - no other thread ever touches it, so no cross-thread ordering is involved.
+__device__ __forceinline__ void tmem_alloc(uint32_t *slot_smem, uint32_t ncols)
+{
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_addr_u32(slot_smem)), "r"(ncols) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t ncols)
+{
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols) : "memory");
+}
+__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+template <int W> __device__ __forceinline__ void tmem_st(uint32_t taddr, const uint32_t (&v)[W]);
+template <> __device__ __forceinline__ void tmem_st<1>(uint32_t taddr, const uint32_t (&v)[1])
+{
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x1.b32 [%0], {%1};" ::"r"(taddr), "r"(v[0]) : "memory");
+}
+template <> __device__ __forceinline__ void tmem_st<2>(uint32_t taddr, const uint32_t (&v)[2])
+{
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1, %2};" ::"r"(taddr), "r"(v[0]), "r"(v[1]) : "memory");
+}
+template <> __device__ __forceinline__ void tmem_st<4>(uint32_t taddr, const uint32_t (&v)[4])
+{
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};" ::"r"(taddr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3])
+                 : "memory");
+}
+// the registers of a tcgen05.ld are valid after tcgen05.wait::ld: the wait names them so that no use moves above it
+template <int W> __device__ __forceinline__ void tmem_ld(uint32_t taddr, uint32_t (&v)[W]);
+template <int W> __device__ __forceinline__ void tmem_wait_ld(uint32_t (&v)[W]);
+template <> __device__ __forceinline__ void tmem_ld<1>(uint32_t taddr, uint32_t (&v)[1])
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x1.b32 {%0}, [%1];" : "=r"(v[0]) : "r"(taddr) : "memory");
+}
+template <> __device__ __forceinline__ void tmem_ld<2>(uint32_t taddr, uint32_t (&v)[2])
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0, %1}, [%2];" : "=r"(v[0]), "=r"(v[1]) : "r"(taddr) : "memory");
+}
+template <> __device__ __forceinline__ void tmem_ld<4>(uint32_t taddr, uint32_t (&v)[4])
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]) : "r"(taddr)
+                 : "memory");
+}
+template <> __device__ __forceinline__ void tmem_wait_ld<1>(uint32_t (&v)[1])
+{
+    asm volatile("tcgen05.wait::ld.sync.aligned;" : "+r"(v[0])::"memory");
+}
+template <> __device__ __forceinline__ void tmem_wait_ld<2>(uint32_t (&v)[2])
+{
+    asm volatile("tcgen05.wait::ld.sync.aligned;" : "+r"(v[0]), "+r"(v[1])::"memory");
+}
+template <> __device__ __forceinline__ void tmem_wait_ld<4>(uint32_t (&v)[4])
+{
+    asm volatile("tcgen05.wait::ld.sync.aligned;" : "+r"(v[0]), "+r"(v[1]), "+r"(v[2]), "+r"(v[3])::"memory");
+}
+
 // ------------------------------------------------------------------ the sweep
 // T: storage/arithmetic type.  R: rows (ROW) and columns (COL) per tile.
 // E: hop entry type.  COL: which sweep.  LZ: Lanczos form.
@@ -405,14 +470,20 @@ gather_sweep_kernel(GatherArgs<T> A)
     const int64_t ld = A.in.ld;
     const T tt = (T)A.t, UU = (T)A.U;
 
-    T ac = T(0), c = T(1), bcp = T(0);
+    // Folded form: line 4's "- b_{j+1} f_j" is applied by the ROW sweep, which has u_j in hand, as
+    // z = (t H_dn + D) w - b_{j+1}^2 f_j  (so that c z = ... - b_{j+1} f_j), with b_{j+1}^2 = |q_j|^2 - a_j^2 known before
+    // the sweep (|w|^2 itself only exists when the sweep ends; the recorded b_{j+1} is still that |w|).  The COL sweep
+    // then reads w and z only.
+    const bool fold = LZ && A.fold_cols > 0;
+    T ac = T(0), c = T(1), bcp = T(0), b2c = T(0);
     if (LZ) {
         if (A.S->stop) return;
         if (!COL) {
             ac = (T)(A.S->alpha * A.S->c_cur);            // line 6: w = q_j - a_j f_j, f_j = c_j u_j
+            if (fold && A.S->started > 0) b2c = (T)((A.S->qnorm2 - A.S->alpha * A.S->alpha) * A.S->c_cur);
         } else {
             c = (T)A.S->c_cur;                            // f_{j+1} = c w
-            bcp = (T)(A.S->beta * A.S->c_prev);           // b_{j+1} f_j = (b_{j+1} c_j) u_j
+            if (!fold) bcp = (T)(A.S->beta * A.S->c_prev);    // b_{j+1} f_j = (b_{j+1} c_j) u_j
         }
     }
     if (!LZ && !COL && A.y_rowmajor && A.S) {
@@ -430,6 +501,7 @@ gather_sweep_kernel(GatherArgs<T> A)
     uint16_t *wsl_s = reinterpret_cast<uint16_t *>(smem_raw + (size_t)(n_in_p + kZeroSlots) * sizeof(PR));
     for (int i = threadIdx.x; i < n_in_w / 32; i += nthr) wsl_s[i] = A.in.wslots[i];   // slots per warp of positions
     double racc = 0.0;                                    // |w|^2 (ROW) or q.f (COL) partial
+    double racc2 = 0.0;                                   // COL: |q|^2 partial
     const int64_t tile_bytes = (int64_t)n_in_p * (int64_t)sizeof(PR);
     // COL stages one contiguous block with no arithmetic on the way: a bulk copy when it is 16-byte granular
     const bool bulk_stage = COL && GS_TMA_STAGE && (tile_bytes % 16) == 0;
@@ -451,6 +523,18 @@ gather_sweep_kernel(GatherArgs<T> A)
 
     using LY = Layout<T, R>;
     constexpr int S = LY::S;
+    // folded ROW sweep: this warp's columns of tensor memory, one piece per gather iteration
+    constexpr int WPP = (int)sizeof(PR) / 4;              // 32-bit columns per piece
+    __shared__ uint32_t tmem_base_s;
+    uint32_t tcol = 0;
+    const bool park = !COL && fold;
+    if (park) {
+        if (wv == 0) tmem_alloc(&tmem_base_s, (uint32_t)A.fold_cols);
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        __syncthreads();
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        tcol = tmem_base_s + (((uint32_t)(wv & 3) * 32u) << 16) + (uint32_t)(wv >> 2) * (uint32_t)(n_it * WPP);
+    }
     // piece of position i of the current tile
     auto poff = [&](int i) { return (int64_t)(i / R) * (S * R) + i % R; };
 
@@ -462,7 +546,33 @@ gather_sweep_kernel(GatherArgs<T> A)
         if (COL || LZ) {
             // tile-major layouts: the pieces are already the interleaved shared-memory image
             const PR *src = reinterpret_cast<const PR *>(COL ? A.Wct : A.Qrt) + tbase;
-            if (!COL) {
+            if (park) {
+                // same thread <-> position map as the gather, so that the piece of u_j parked here is this thread's
+                // own in the epilogue (whole warps: the tensor-memory accesses are warp-collective)
+                const PR *fsrc = reinterpret_cast<const PR *>(A.Frt) + tbase;
+                PR *wdst = reinterpret_cast<PR *>(A.Qrt) + tbase;
+                for (int it = 0; it < n_it; ++it) {
+                    const int i = pos_of(it);
+                    if (i >= n_in_w) continue;
+                    PR v, f;
+#pragma unroll
+                    for (int r = 0; r < R; ++r) v.v[r] = f.v[r] = T(0);
+                    if (i < n_in_p) { v = ld_once<1>(src + poff(i)); f = ld_once<1>(fsrc + poff(i)); }
+#pragma unroll
+                    for (int r = 0; r < R; ++r) {
+                        v.v[r] = v.v[r] - ac * f.v[r];
+                        racc += (double)v.v[r] * (double)v.v[r];
+                    }
+                    if (i < n_in_p) {
+                        st_once<1>(wdst + poff(i), v);
+                        Xs[i] = v;
+                    }
+                    uint32_t fw[WPP];
+                    memcpy(fw, &f, sizeof(PR));
+                    tmem_st<WPP>(tcol + (uint32_t)(it * WPP), fw);
+                }
+                tmem_wait_st();
+            } else if (!COL) {
                 const PR *fsrc = reinterpret_cast<const PR *>(A.Frt) + tbase;
                 PR *wdst = reinterpret_cast<PR *>(A.Qrt) + tbase;
                 // loads of kStageUnroll pieces are issued before the first store (w overwrites q in place)
@@ -543,12 +653,14 @@ gather_sweep_kernel(GatherArgs<T> A)
             PR z, f;
 #pragma unroll
             for (int r = 0; r < R; ++r) z.v[r] = f.v[r] = T(0);
+            uint32_t fw[WPP];
 #if GS_HOIST
             if (!COL) {
                 if (valid) sd = A.in.st[i];
+                if (park && !GS_FOLD_LATE) tmem_ld<WPP>(tcol + (uint32_t)(it * WPP), fw);
             } else if (inpad) {
                 z = ld_once<(sizeof(T) == 4 ? 4 : 8)>(reinterpret_cast<const PR *>(A.Zct) + tbase + poff(i));
-                if (LZ) f = ld_once<(sizeof(T) == 4 ? 4 : 8)>(reinterpret_cast<const PR *>(A.Fct) + tbase + poff(i));
+                if (LZ && !fold) f = ld_once<(sizeof(T) == 4 ? 4 : 8)>(reinterpret_cast<const PR *>(A.Fct) + tbase + poff(i));
             }
 #endif
             // keep DRAM busy during the gather: a slice of the next tile's inputs goes to L2 every iteration
@@ -595,9 +707,10 @@ gather_sweep_kernel(GatherArgs<T> A)
 #if !GS_HOIST
             if (!COL) {
                 if (valid) sd = A.in.st[i];
+                if (park && !GS_FOLD_LATE) tmem_ld<WPP>(tcol + (uint32_t)(it * WPP), fw);
             } else if (inpad) {
                 z = ld_once<(sizeof(T) == 4 ? 4 : 8)>(reinterpret_cast<const PR *>(A.Zct) + tbase + poff(i));
-                if (LZ) f = ld_once<(sizeof(T) == 4 ? 4 : 8)>(reinterpret_cast<const PR *>(A.Fct) + tbase + poff(i));
+                if (LZ && !fold) f = ld_once<(sizeof(T) == 4 ? 4 : 8)>(reinterpret_cast<const PR *>(A.Fct) + tbase + poff(i));
             }
 #endif
             const int q = i % R;
@@ -608,6 +721,13 @@ gather_sweep_kernel(GatherArgs<T> A)
                 T h[R];
 #pragma unroll
                 for (int r = 0; r < R; ++r) h[r] = tt * acc[r] + UU * (T)__popc(so[r] & sd) * xi.v[r];
+                if (park) {
+                    if (GS_FOLD_LATE) tmem_ld<WPP>(tcol + (uint32_t)(it * WPP), fw);
+                    tmem_wait_ld<WPP>(fw);
+                    memcpy(&f, fw, sizeof(PR));
+#pragma unroll
+                    for (int r = 0; r < R; ++r) h[r] -= b2c * f.v[r];          // - b_{j+1}^2 f_j (line 4, eq. 13)
+                }
                 if (!LZ && A.y_rowmajor) {
                     // hubbard_apply, hybrid form: y = (t H_dn + D) x in the caller's row-major layout
                     // (coalesced over i for each of the R rows); the strip sweep adds the up term
@@ -634,6 +754,7 @@ gather_sweep_kernel(GatherArgs<T> A)
                     for (int r = 0; r < R; ++r) {
                         qv[r] = c * (tt * acc[r] + z.v[r]) - bcp * f.v[r];      // line 4 + eq. 13
                         racc += (double)qv[r] * (double)(c * xi.v[r]);          // line 5
+                        racc2 += (double)qv[r] * (double)qv[r];
                     }
                     const PR qt = block_transpose<T, R>(qv, q);
                     if (inpad) st_once<4>(outZ + oidx, qt);
@@ -648,15 +769,27 @@ gather_sweep_kernel(GatherArgs<T> A)
         }
     }
 
+    if (park) {
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        __syncthreads();
+        if (wv == 0) tmem_dealloc(tmem_base_s, (uint32_t)A.fold_cols);
+    }
     if (LZ) {
         const double sblk = block_sum(racc, red);
+        if (COL) {
+            // second partial of the block, published by the same ticket (thread 0 writes both before its fence)
+            const double sblk2 = block_sum(racc2, red);
+            if (threadIdx.x == 0) A.partials[gridDim.x + blockIdx.x] = sblk2;
+        }
         if (publish_and_check_last(sblk, A.partials, blockIdx.x, gridDim.x, &A.S->ticket, &flag)) {
             const double tot = sum_partials(A.partials, gridDim.x, red);
-            if (threadIdx.x == 0) {
-                if (!COL) {
-                    lanczos_rotate(A.S, tot, A.alpha_out, A.beta_out);
-                } else {
+            if (!COL) {
+                if (threadIdx.x == 0) lanczos_rotate(A.S, tot, A.alpha_out, A.beta_out);
+            } else {
+                const double tot2 = sum_partials(A.partials + gridDim.x, gridDim.x, red);
+                if (threadIdx.x == 0) {
                     A.S->alpha = tot;
+                    A.S->qnorm2 = tot2;
                     A.S->ticket = 0;
                 }
             }
@@ -739,7 +872,7 @@ from_rt_kernel(const T *__restrict__ rt, T *__restrict__ x, int64_t du, int64_t 
 __global__ void lanczos_scalars_init_kernel(LanczosScalars *S, double tau)
 {
     S->c_cur = 0.0; S->c_prev = 0.0; S->beta = 0.0; S->alpha = 0.0; S->amax = 0.0; S->tau = tau;
-    S->j = 0; S->stop = 0; S->ticket = 0; S->started = 0;
+    S->j = 0; S->stop = 0; S->ticket = 0; S->started = 0; S->qnorm2 = 0.0;
 }
 
 }  // namespace hub

@@ -409,6 +409,39 @@ def test_lanczos_C5_free_fermions(dtype):
 
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("ctas", [1, 2, 4])
+@pytest.mark.parametrize("name,ns,nu,nd,bonds", [("C2", 12, 6, 6, ring_bonds(12)), ("odd", 13, 5, 7, ring_bonds(13) + [(0, 5)])])
+def test_gather_lanczos_folded_and_nine_pass_forms(name, ns, nu, nd, bonds, ctas, dtype):
+    """Variant GATHER has two Lanczos forms: the folded one (default: the ROW sweep parks its tile of
+    u_j in tensor memory and applies line 4's - b_{j+1} f_j itself, with b_{j+1}^2 = |q_j|^2 - a_j^2 from the COL
+    sweep before; 8 vector passes) and the nine-pass one (gather_fold = 0: the COL sweep reads u_j).  Both against
+    Algorithm 1 of the oracle, with 1, 2 and 4 CTAs per SM sharing the SM's 512 tensor-memory columns."""
+    ref = RefModel(ns, nu, nd, bonds, 1.0, 4.0)
+    x, x_np = start_vector(78, ref.dim, dtype)
+    a_ref, b_ref = lr.lanczos(ref.apply, x_np, 40)
+    e_ref = lr.ground_energy(a_ref, b_ref)
+    tol_c = 1e-10 if dtype == "f64" else 1e-5
+    got = {}
+    for fold in (1, 0):
+        m = hb.hubbard_create(ns, nu, nd, bonds, 1.0, 4.0, dtype)
+        m.hubbard_set_variant(hb.VARIANT_GATHER)
+        m.hubbard_debug_set("gather_ctas", ctas)
+        m.hubbard_debug_set("gather_fold", fold)
+        cols = m.hubbard_debug_get("resolved_gather_fold")
+        assert (cols >= 32 and cols & (cols - 1) == 0 and cols * ctas <= 512) if fold else cols == 0
+        alpha, beta = m.lanczos_run(x, 40)
+        n = 30
+        assert np.max(np.abs(alpha[:n] - a_ref[:n]) / np.maximum(1.0, np.abs(a_ref[:n]))) <= tol_c
+        assert np.max(np.abs(beta[:n] - b_ref[:n]) / np.maximum(1.0, np.abs(b_ref[:n]))) <= tol_c
+        assert abs(hb.lanczos_ground_energy(alpha, beta) - e_ref) <= TOL_E0[dtype] * abs(e_ref)
+        a2, b2 = m.lanczos_run(x, 40)
+        assert np.array_equal(alpha, a2) and np.array_equal(beta, b2)      # deterministic, and tensor memory is released
+        got[fold] = (alpha, beta)
+    # the two forms differ only in rounding (the coefficient of f_j is |q|^2 - a^2 instead of |w|^2)
+    assert np.max(np.abs(got[0][0][:30] - got[1][0][:30])) <= tol_c * 20
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
 @pytest.mark.parametrize("name,ns,nu,nd,bonds", [("C2", 12, 6, 6, ring_bonds(12)), ("odd", 13, 5, 7, ring_bonds(13) + [(0, 5)])])
 def test_auto_twosweep_with_gather_row(name, ns, nu, nd, bonds, dtype):
     """The path C5 fp32 takes under AUTO, on sectors the oracle covers in full: the gather tile is narrower than
