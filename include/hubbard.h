@@ -318,9 +318,11 @@ int64_t hubbard_launch_count(const hubbard_model *m);
  *   "gather_nosort" (0/1)     the Lanczos work vectors of variant GATHER keep the basis order
  *   "gather_nosymmetry" (0/1) their internal order comes from hop counts only (no lattice-symmetry orbits)
  *   "gather_ctas" (1-4)       CTAs per SM for small tiles
- *   "gather_fold" (0/1)       1 (default): lanczos_* of variant GATHER in the folded, eight-pass form (the ROW sweep parks
- *                             its tile of u_j in tensor memory and applies "- b_{j+1} f_j" of Algorithm 1 line 4 itself);
- *                             0: the nine-pass form (the COL sweep reads u_j).  DESIGN.md 2 (readings) and 4.2
+ *   "gather_fold" (0-2)       lanczos_* of variant GATHER in the folded, eight-pass form (the ROW sweep parks its tile of
+ *                             u_j in tensor memory and applies "- b_{j+1} f_j" of Algorithm 1 line 4 itself): 1 (default)
+ *                             where one tile fills an SM's shared memory (C4), 2 wherever the SM's 512 tensor-memory
+ *                             columns suffice for its resident CTAs, 0 never = the nine-pass form (the COL sweep reads
+ *                             u_j).  DESIGN.md 2 (readings) and 4.2
  *   "apply_pure_gather" (0/1) plain hubbard_apply as two gather sweeps instead of the hybrid
  *   "twosweep_old_row" (0/1)  AUTO's TWOSWEEP fallback keeps the first row kernel
  *   "row_R" (0-4), "strip_mb" (1-1024), "strip_rb"   geometry of variant TWOSWEEP (0 = automatic)

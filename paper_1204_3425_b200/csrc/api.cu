@@ -347,16 +347,20 @@ void gather_launch_shape(const hubbard_model *m, size_t smem, int *per_sm, int *
 
 // Folded Lanczos form of variant GATHER: tensor-memory columns one CTA of the ROW sweep needs to park its tile of u_j
 // (one 16-byte piece per thread and gather iteration; a warp addresses a quarter of the 128 lanes), as the power of
-// two >= 32 that tcgen05.alloc takes.  0: the nine-pass form (knob off, or the resident CTAs of an SM would need more
-// than its 512 columns).
+// two >= 32 that tcgen05.alloc takes.  0: the nine-pass form (knob 0; knob 1 = automatic and several CTAs per SM; or the
+// resident CTAs of an SM would need more than its 512 columns).  Knob 2 folds wherever the columns suffice.
 int gather_fold_cols(const hubbard_model *m)
 {
     const int R = gather_R(m);
     if (!m->opt.gather_fold || R == 0) return 0;
     const size_t es = m->dtype == HUBBARD_F32 ? 4 : 8;
+    if (R * es != 16) return 0;          // full-width tiles only (what AUTO runs as GATHER; narrower ones are test geometry)
     const int64_t dd_p = round_up(m->dn.dim, gather_align(m));
     int per_sm, threads;
     gather_launch_shape(m, gather_smem_bytes(dd_p, R, es), &per_sm, &threads);
+    // automatic: only where one tile fills the SM (C4).  Measured with the fold forced: C3 (2 CTAs per SM) no gain
+    // (ROW + COL 0.376 ms either way), C2 (4 CTAs per SM, 4 tiles each) 10 % slower (the allocation is per launch).
+    if (m->opt.gather_fold == 1 && per_sm != 1) return 0;
     const int64_t n_it = (round_up(dd_p, 32) + threads - 1) / threads;
     const int64_t need = (int64_t)((threads / 32 + 3) / 4) * n_it * (int64_t)(R * es / 4);
     int64_t cols = 32;
@@ -364,10 +368,10 @@ int gather_fold_cols(const hubbard_model *m)
     return (cols * per_sm <= 512) ? (int)cols : 0;
 }
 
-template <typename T, int R, typename E, bool COL, bool LZ>
-int launch_gather_inst(hubbard_model *m, GatherArgs<T> A, cudaStream_t st)
+template <typename T, int R, typename E, bool COL, bool LZ, bool FOLD>
+int launch_gather_fold(hubbard_model *m, GatherArgs<T> A, cudaStream_t st)
 {
-    auto kern = gather_sweep_kernel<T, R, E, COL, LZ>;
+    auto kern = gather_sweep_kernel<T, R, E, COL, LZ, FOLD>;
     A.du_p = round_up(A.dim_up, gather_align(m));
     A.dd_p = round_up(A.dim_dn, gather_align(m));
     const int64_t n_in_p = COL ? A.du_p : A.dd_p;
@@ -382,6 +386,16 @@ int launch_gather_inst(hubbard_model *m, GatherArgs<T> A, cudaStream_t st)
         kern<<<grid, threads, smem, st>>>(A);
     }
     return after_launch(m);
+}
+
+template <typename T, int R, typename E, bool COL, bool LZ>
+int launch_gather_inst(hubbard_model *m, GatherArgs<T> A, cudaStream_t st)
+{
+    if constexpr (LZ && sizeof(E) == 2) {
+        if (A.fold_cols > 0) return launch_gather_fold<T, R, E, COL, LZ, true>(m, A, st);
+    }
+    A.fold_cols = 0;
+    return launch_gather_fold<T, R, E, COL, LZ, false>(m, A, st);
 }
 
 // LZ: the Lanczos sweeps work in the sorted internal order of BOTH spins; plain apply (row-major callers) in basis order.
@@ -1427,7 +1441,7 @@ const OptKey kOptKeys[] = {
     {"gather_nosort", &hub::DebugOptions::gather_nosort, true, 0, 1},
     {"gather_nosymmetry", &hub::DebugOptions::gather_nosymmetry, true, 0, 1},
     {"gather_ctas", &hub::DebugOptions::gather_ctas, false, 1, 4},
-    {"gather_fold", &hub::DebugOptions::gather_fold, false, 0, 1},
+    {"gather_fold", &hub::DebugOptions::gather_fold, false, 0, 2},
     {"apply_pure_gather", &hub::DebugOptions::apply_pure_gather, false, 0, 1},
     {"twosweep_old_row", &hub::DebugOptions::twosweep_old_row, false, 0, 1},
     {"row_R", &hub::DebugOptions::row_R, false, 0, 4},

@@ -445,10 +445,14 @@ template <> __device__ __forceinline__ void tmem_wait_ld<4>(uint32_t (&v)[4])
 // ------------------------------------------------------------------ the sweep
 // T: storage/arithmetic type.  R: rows (ROW) and columns (COL) per tile.
 // E: hop entry type.  COL: which sweep.  LZ: Lanczos form.
-template <typename T, int R, typename E, bool COL, bool LZ>
+// FOLD: the folded (eight-pass) Lanczos form.  It is an instantiation of its own because a kernel that merely CONTAINS
+// tcgen05.alloc is scheduled differently (its CTAs hold the SM's allocation permit from launch): the
+// nine-pass kernels have no tensor-memory instruction in them.
+template <typename T, int R, typename E, bool COL, bool LZ, bool FOLD = false>
 __global__ void __launch_bounds__(kGatherMaxThreads, 1)
 gather_sweep_kernel(GatherArgs<T> A)
 {
+    static_assert(LZ || !FOLD, "the fold is a Lanczos form");
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ double red[32];
     __shared__ int flag;
@@ -474,7 +478,7 @@ gather_sweep_kernel(GatherArgs<T> A)
     // z = (t H_dn + D) w - b_{j+1}^2 f_j  (so that c z = ... - b_{j+1} f_j), with b_{j+1}^2 = |q_j|^2 - a_j^2 known before
     // the sweep (|w|^2 itself only exists when the sweep ends; the recorded b_{j+1} is still that |w|).  The COL sweep
     // then reads w and z only.
-    const bool fold = LZ && A.fold_cols > 0;
+    constexpr bool fold = FOLD;
     T ac = T(0), c = T(1), bcp = T(0), b2c = T(0);
     if (LZ) {
         if (A.S->stop) return;
@@ -527,7 +531,7 @@ gather_sweep_kernel(GatherArgs<T> A)
     constexpr int WPP = (int)sizeof(PR) / 4;              // 32-bit columns per piece
     __shared__ uint32_t tmem_base_s;
     uint32_t tcol = 0;
-    const bool park = !COL && fold;
+    constexpr bool park = !COL && fold;
     if (park) {
         if (wv == 0) tmem_alloc(&tmem_base_s, (uint32_t)A.fold_cols);
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
@@ -754,7 +758,7 @@ gather_sweep_kernel(GatherArgs<T> A)
                     for (int r = 0; r < R; ++r) {
                         qv[r] = c * (tt * acc[r] + z.v[r]) - bcp * f.v[r];      // line 4 + eq. 13
                         racc += (double)qv[r] * (double)(c * xi.v[r]);          // line 5
-                        racc2 += (double)qv[r] * (double)qv[r];
+                        if (fold) racc2 += (double)qv[r] * (double)qv[r];
                     }
                     const PR qt = block_transpose<T, R>(qv, q);
                     if (inpad) st_once<4>(outZ + oidx, qt);
@@ -776,7 +780,7 @@ gather_sweep_kernel(GatherArgs<T> A)
     }
     if (LZ) {
         const double sblk = block_sum(racc, red);
-        if (COL) {
+        if (COL && fold) {
             // second partial of the block, published by the same ticket (thread 0 writes both before its fence)
             const double sblk2 = block_sum(racc2, red);
             if (threadIdx.x == 0) A.partials[gridDim.x + blockIdx.x] = sblk2;
@@ -786,7 +790,7 @@ gather_sweep_kernel(GatherArgs<T> A)
             if (!COL) {
                 if (threadIdx.x == 0) lanczos_rotate(A.S, tot, A.alpha_out, A.beta_out);
             } else {
-                const double tot2 = sum_partials(A.partials + gridDim.x, gridDim.x, red);
+                const double tot2 = fold ? sum_partials(A.partials + gridDim.x, gridDim.x, red) : 0.0;
                 if (threadIdx.x == 0) {
                     A.S->alpha = tot;
                     A.S->qnorm2 = tot2;

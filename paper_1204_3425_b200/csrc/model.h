@@ -24,11 +24,11 @@ struct LanczosScalars {
     double alpha;    // a_j of the iteration in flight
     double amax;     // max_k |a_k| so far (breakdown rule, reading Q11)
     double tau;
-    double qnorm2;   // |q_j|^2 of the iteration in flight (variant GATHER, folded form: b_{j+1}^2 = |q_j|^2 - a_j^2 ahead of the ROW sweep)
     int j;           // iterations completed
     int stop;        // breakdown (or bad start vector): later sweeps are no-ops
     unsigned ticket; // arrival counter of the sweep in flight
     int started; // norm-producing sweeps finished (variant GATHER)
+    double qnorm2;   // |q_j|^2 of the iteration in flight (variant GATHER, folded form: b_{j+1}^2 = |q_j|^2 - a_j^2 ahead of the ROW sweep)
 };
 
 // One spin's hop table in the device layout of variant GATHER (gather_tables.h): batch-interleaved ELL over the
@@ -80,7 +80,8 @@ struct DebugOptions {
     int gather_nosort = 0;          // 1: the Lanczos work vectors keep the basis order (no internal reordering)
     int gather_nosymmetry = 0;      // 1: internal order from hop counts only (no lattice-symmetry orbits)
     int gather_ctas = 4;            // CTAs per SM for small tiles
-    int gather_fold = 1;            // 1: eight-pass Lanczos form (- b f_{j-1} folded into the ROW sweep through tensor memory)
+    int gather_fold = 1;            // eight-pass Lanczos form (- b f_{j-1} folded into the ROW sweep through tensor memory):
+                                    // 0 never, 1 where one tile fills the SM (automatic), 2 wherever the tensor memory suffices
     int apply_pure_gather = 0;      // 1: plain hubbard_apply as two gather sweeps instead of the hybrid
     int twosweep_old_row = 0;       // 1: TWOSWEEP fallback keeps the first row kernel
     int row_R = 0;                  // rows per CTA of the TWOSWEEP row kernel (0 = automatic)

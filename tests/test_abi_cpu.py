@@ -268,10 +268,10 @@ def test_debug_knobs_are_explicit_per_model_state(monkeypatch):
     assert m.hubbard_debug_get("gather_R") == 2
     m2 = hb.hubbard_create_host(c.n_sites, c.n_up, c.n_dn, c.bonds, c.t, 4.0)
     assert m2.hubbard_debug_get("gather_R") == 0         # no process-wide state
-    assert m.hubbard_debug_get("gather_fold") == 1       # eight-pass Lanczos form is the default
+    assert m.hubbard_debug_get("gather_fold") == 1       # eight-pass Lanczos form: automatic (where one tile fills the SM)
     m.hubbard_debug_set("gather_fold", 0)
     assert m.hubbard_debug_get("gather_fold") == 0 and m.hubbard_debug_get("resolved_gather_fold") == 0
-    for key, bad in (("gather_R", 5), ("gather_ctas", 0), ("no_such_key", 1), ("cluster_NC", -1), ("gather_fold", 2)):
+    for key, bad in (("gather_R", 5), ("gather_ctas", 0), ("no_such_key", 1), ("cluster_NC", -1), ("gather_fold", 3)):
         with pytest.raises(hb.HubbardError):
             m.hubbard_debug_set(key, bad)
     with pytest.raises(hb.HubbardError):
