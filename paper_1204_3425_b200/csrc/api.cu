@@ -141,7 +141,12 @@ int upload_gather_table(hubbard_model *m, const SpinTable &tab, int R, int align
     G.e16 = nullptr;
     if (T.n_pos + 128 <= 32768) {
         std::vector<uint16_t> e16(T.ent.size());
-        for (size_t i = 0; i < T.ent.size(); ++i) e16[i] = (uint16_t)T.ent[i];
+        // device form of the 16-bit entries (kernels_gather.cuh, hop_lo / hop_hi): even slots position << 1 | neg,
+        // odd slots position | neg << 15 (a slot's parity is its index's: batches are 8 entries)
+        for (size_t i = 0; i < T.ent.size(); ++i) {
+            const uint32_t pos = T.ent[i] >> 1, neg = T.ent[i] & 1u;
+            e16[i] = (uint16_t)((i & 1) ? (pos | (neg << 15)) : ((pos << 1) | neg));
+        }
         if ((rc = dev_upload(m, e16, &G.e16, true))) return rc;
     }
     *out = G;

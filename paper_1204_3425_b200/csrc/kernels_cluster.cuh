@@ -37,7 +37,7 @@ row_cluster_kernel(ClusterRowArgs<T> A)
     cg::cluster_group cluster = cg::this_cluster();
     extern __shared__ __align__(16) unsigned char smem_raw[];
     using PR = Pack<T, R>;
-    using EB = Pack<E, kGatherBatch>;
+    using EB = typename BatchOf<E>::type;
     PR *Xs = reinterpret_cast<PR *>(smem_raw);            // [my_n + kZero]
     constexpr int kZero = 128 / (int)sizeof(PR);          // zero slots, one per bank group (padding entries)
 
@@ -100,8 +100,15 @@ row_cluster_kernel(ClusterRowArgs<T> A)
                 const EB nxt = load_batch(np);
 #pragma unroll
                 for (int j = 0; j < kGatherBatch; ++j) {
-                    const uint32_t e = pk.v[j];
-                    const int col = (int)(e >> 1);
+                    int col;
+                    T s;
+                    if constexpr (sizeof(E) == 2) {      // packed 16-bit device entries (kernels_gather.cuh)
+                        col = (int)packed_pos(pk, j);
+                        s = packed_sign<T>(pk, j);
+                    } else {
+                        col = (int)(pk.v[j] >> 1);
+                        s = sign_one<T>(pk.v[j]);
+                    }
                     // one branch-free generic load: the owner's part (this CTA's own or another's through
                     // distributed shared memory), or a local zero slot for a padding entry
                     int owner = 0;
@@ -113,7 +120,6 @@ row_cluster_kernel(ClusterRowArgs<T> A)
                     const PR *src = ob + (col - owner * part);
                     src = (col >= dd) ? Xs + my_n + (col - zero_base) : src;
                     const PR v = *src;
-                    const T s = sign_one<T>(e);
 #pragma unroll
                     for (int r = 0; r < R; ++r) acc[r] = fma(s, v.v[r], acc[r]);
                 }

@@ -125,11 +125,15 @@ template <> __device__ __forceinline__ double sign_one<double>(uint32_t e)
 
 // One batch of kGatherBatch hop entries of one state: contiguous bytes, read
 // through the read-only path with the widest loads.
-template <typename E>
-__device__ __forceinline__ Pack<E, kGatherBatch> load_batch(const Pack<E, kGatherBatch> *p)
+// (16-bit entries travel as the four 32-bit words they are packed in - a struct of eight uint16 makes the compiler
+// re-pack them with PRMT at every copy.)
+template <typename E> struct BatchOf { using type = Pack<E, kGatherBatch>; };
+template <> struct BatchOf<uint16_t> { using type = Pack<uint32_t, kGatherBatch / 2>; };
+template <typename E, int N>
+__device__ __forceinline__ Pack<E, N> load_batch(const Pack<E, N> *p)
 {
-    constexpr int kBytes = (int)sizeof(E) * kGatherBatch;
-    Pack<E, kGatherBatch> o;
+    constexpr int kBytes = (int)sizeof(E) * N;
+    Pack<E, N> o;
     if constexpr (kBytes % 16 == 0) {
         uint4 u[kBytes / 16];
 #pragma unroll
@@ -314,50 +318,103 @@ __device__ __forceinline__ void hop(const unsigned char *xs_bytes, uint32_t e, T
     for (int r = 0; r < R; ++r) acc[r] = fma(s, v.v[r], acc[r]);
 }
 
-// ---- hop entries straight from the packed 32-bit words of a batch (uint16 entries: two per word), without
-// unpacking them first: byte offset of entry e = (e & ~1) * sizeof(PR) / 2, sign = bit 0.
+// ---- 16-bit device entries, two per 32-bit word (upload_gather_table): the EVEN entry of a word as
+// position << 1 | neg in bits 0..15, the ODD one as position | neg << 15 in bits 16..31 (the matrix element is
+// t * (neg ? -1 : +1)).  Chosen for what one integer instruction can do: the byte offset of either
+// entry is one mask and one shift-and-add away from the word (LOP3 + LEA / LEA.HI), the sign of the odd entry is
+// already where a float / the high word of a double has it, the sign of the even one is one shift-and-add (w << 31).
+template <typename PR>
+__device__ __forceinline__ PR lds_piece(uint32_t saddr)
+{
+    PR v;
+    if constexpr (sizeof(PR) == 16) {
+        uint32_t a, b, c, d;
+        asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(a), "=r"(b), "=r"(c), "=r"(d) : "r"(saddr));
+        const uint32_t u[4] = {a, b, c, d};
+        memcpy(&v, u, 16);
+    } else if constexpr (sizeof(PR) == 8) {
+        uint32_t a, b;
+        asm volatile("ld.shared.v2.b32 {%0, %1}, [%2];" : "=r"(a), "=r"(b) : "r"(saddr));
+        const uint32_t u[2] = {a, b};
+        memcpy(&v, u, 8);
+    } else {
+        static_assert(sizeof(PR) == 4, "pieces are 4, 8 or 16 bytes");
+        uint32_t a;
+        asm volatile("ld.shared.b32 %0, [%1];" : "=r"(a) : "r"(saddr));
+        memcpy(&v, &a, 4);
+    }
+    return v;
+}
+template <typename T> __device__ __forceinline__ T sign_top(uint32_t w);      // +-1 from bit 31
+template <> __device__ __forceinline__ float sign_top<float>(uint32_t w) { return __uint_as_float((w & 0x80000000u) | 0x3f800000u); }
+template <> __device__ __forceinline__ double sign_top<double>(uint32_t w)
+{
+    return __hiloint2double((int)((w & 0x80000000u) | 0x3ff00000u), 0);
+}
 template <typename T, int R>
-__device__ __forceinline__ void hop_lo(const unsigned char *xs_bytes, uint32_t w, T (&acc)[R])      // entry in bits 0..15
+__device__ __forceinline__ void hop_lo(uint32_t xs_s, uint32_t w, T (&acc)[R])      // even entry: bits 0..15
 {
     using PR = Pack<T, R>;
     constexpr int SH = sizeof(PR) == 16 ? 3 : sizeof(PR) == 8 ? 2 : 1;
-    const PR v = *reinterpret_cast<const PR *>(xs_bytes + ((w << SH) & (0xfffeu << SH)));
+    const PR v = lds_piece<PR>(xs_s + ((w & 0xfffeu) << SH));
     const T s = sign_one<T>(w);                            // (w << 31): only bit 0 survives
 #pragma unroll
     for (int r = 0; r < R; ++r) acc[r] = fma(s, v.v[r], acc[r]);
 }
 template <typename T, int R>
-__device__ __forceinline__ void hop_hi(const unsigned char *xs_bytes, uint32_t w, T (&acc)[R])      // entry in bits 16..31
+__device__ __forceinline__ void hop_hi(uint32_t xs_s, uint32_t w, T (&acc)[R])      // odd entry: bits 16..31
 {
     using PR = Pack<T, R>;
-    constexpr int SH = sizeof(PR) == 16 ? 3 : sizeof(PR) == 8 ? 2 : 1;
-    const PR v = *reinterpret_cast<const PR *>(xs_bytes + ((w >> (16 - SH)) & (0xfffeu << SH)));
-    const T s = sign_one<T>(w >> 16);
+    constexpr int SH = sizeof(PR) == 16 ? 12 : sizeof(PR) == 8 ? 13 : 14;
+    const PR v = lds_piece<PR>(xs_s + ((w & 0x7fff0000u) >> SH));
+    if constexpr (sizeof(T) == 8) {
+        // the sign bit of the entry IS the sign bit of a double's high word: flip it into the value (one three-input
+        // LOP3 per output) and add - no +-1.0 to build, exact like the multiplication by +-1
 #pragma unroll
-    for (int r = 0; r < R; ++r) acc[r] = fma(s, v.v[r], acc[r]);
+        for (int r = 0; r < R; ++r)
+            acc[r] += __hiloint2double(__double2hiint(v.v[r]) ^ (int)(w & 0x80000000u), __double2loint(v.v[r]));
+    } else {
+        const T s = sign_top<T>(w);
+#pragma unroll
+        for (int r = 0; r < R; ++r) acc[r] = fma(s, v.v[r], acc[r]);
+    }
+}
+// position and sign of entry j of a packed batch, for kernels that do not gather from a local tile
+__device__ __forceinline__ uint32_t packed_pos(const Pack<uint32_t, kGatherBatch / 2> &pk, int j)
+{
+    const uint32_t w = pk.v[j >> 1];
+    return (j & 1) ? ((w >> 16) & 0x7fffu) : ((w >> 1) & 0x7fffu);
+}
+template <typename T>
+__device__ __forceinline__ T packed_sign(const Pack<uint32_t, kGatherBatch / 2> &pk, int j)
+{
+    const uint32_t w = pk.v[j >> 1];
+    return (j & 1) ? sign_top<T>(w) : sign_one<T>(w);
 }
 
 // `count` (warp-uniform, 1..8) entries of a batch.
 template <typename T, int R>
-__device__ __forceinline__ void hop_batch_n(const unsigned char *xs_bytes, const Pack<uint16_t, kGatherBatch> &pk, int count, T (&acc)[R])
+__device__ __forceinline__ void hop_batch_n(const unsigned char *xs_bytes, const Pack<uint32_t, kGatherBatch / 2> &pk, int count, T (&acc)[R])
 {
     static_assert(kGatherBatch == 8, "a batch is four 32-bit words of two entries");
+    const uint32_t xs_s = smem_addr_u32(xs_bytes);
     uint32_t w[4];
-    memcpy(w, &pk, 16);
+#pragma unroll
+    for (int k = 0; k < 4; ++k) w[k] = pk.v[k];
     if (count == kGatherBatch) {
 #pragma unroll
-        for (int k = 0; k < 4; ++k) { hop_lo<T, R>(xs_bytes, w[k], acc); hop_hi<T, R>(xs_bytes, w[k], acc); }
+        for (int k = 0; k < 4; ++k) { hop_lo<T, R>(xs_s, w[k], acc); hop_hi<T, R>(xs_s, w[k], acc); }
     } else {
         if (count & 4) {
-            hop_lo<T, R>(xs_bytes, w[0], acc); hop_hi<T, R>(xs_bytes, w[0], acc);
-            hop_lo<T, R>(xs_bytes, w[1], acc); hop_hi<T, R>(xs_bytes, w[1], acc);
+            hop_lo<T, R>(xs_s, w[0], acc); hop_hi<T, R>(xs_s, w[0], acc);
+            hop_lo<T, R>(xs_s, w[1], acc); hop_hi<T, R>(xs_s, w[1], acc);
             w[0] = w[2]; w[1] = w[3];
         }
         if (count & 2) {
-            hop_lo<T, R>(xs_bytes, w[0], acc); hop_hi<T, R>(xs_bytes, w[0], acc);
+            hop_lo<T, R>(xs_s, w[0], acc); hop_hi<T, R>(xs_s, w[0], acc);
             w[0] = w[1];
         }
-        if (count & 1) hop_lo<T, R>(xs_bytes, w[0], acc);
+        if (count & 1) hop_lo<T, R>(xs_s, w[0], acc);
     }
 }
 template <typename T, int R>
@@ -458,7 +515,7 @@ gather_sweep_kernel(GatherArgs<T> A)
     __shared__ int flag;
     __shared__ __align__(8) uint64_t stage_bar;           // COL: bytes of the bulk-staged tile that have landed
     using PR = Pack<T, R>;
-    using EB = Pack<E, kGatherBatch>;
+    using EB = typename BatchOf<E>::type;
     PR *Xs = reinterpret_cast<PR *>(smem_raw);            // [n_in_p + kZeroSlots]
     constexpr int kZeroSlots = 128 / (int)sizeof(PR);     // lanes served by one shared-memory wavefront
     const unsigned char *xs_bytes = smem_raw;

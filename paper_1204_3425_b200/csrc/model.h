@@ -41,7 +41,8 @@ struct SpinDev {
     int64_t ld;             // positions per batch plane (multiple of 32): entry k of position p
                             // sits at [((k / 8) * ld + p) * 8 + k % 8]
     int w;                  // slots per position in the table (multiple of 8)
-    const uint16_t *e16;    // entries when n_pos + 128 <= 32768, else null
+    const uint16_t *e16;    // when n_pos + 128 <= 32768, else null: the entries in 16 bits - even slots as in e32,
+                            // odd slots as target_position | neg << 15 (what the packed-word decode wants)
     const uint32_t *e32;    // entries (always present)
     const uint16_t *wslots; // per warp of 32 positions: slots every lane of that warp walks (exact)
     const int32_t *perm;    // position -> state index in the basis order of PAPER.md:63-67 (-1: padding)
