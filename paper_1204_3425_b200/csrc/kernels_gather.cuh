@@ -108,6 +108,7 @@ struct Layout {
     static constexpr int S = 1;
     static __host__ __device__ __forceinline__ int64_t piece(int64_t tile, int64_t pos, int64_t n_p)
     {
+        if constexpr (S == 1) return tile * n_p + pos;       // (R divides n_p: the general form below reduces to this)
         return (((tile / S) * (n_p / R) + pos / R) * S + tile % S) * R + pos % R;
     }
 };
@@ -597,7 +598,7 @@ gather_sweep_kernel(GatherArgs<T> A)
         tcol = tmem_base_s + (((uint32_t)(wv & 3) * 32u) << 16) + (uint32_t)(wv >> 2) * (uint32_t)(n_it * WPP);
     }
     // piece of position i of the current tile
-    auto poff = [&](int i) { return (int64_t)(i / R) * (S * R) + i % R; };
+    auto poff = [&](int i) { return S == 1 ? (int64_t)i : (int64_t)(i / R) * (S * R) + i % R; };
 
     for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
         const int64_t o0 = tile * R;
@@ -750,7 +751,16 @@ gather_sweep_kernel(GatherArgs<T> A)
             // batch of this thread's next state
             const EB *ep = reinterpret_cast<const EB *>(ent) + i;
             const int nb = (n + kGatherBatch - 1) / kGatherBatch;
-            for (int b = 0; b + 1 < nb; ++b) {
+            int b = 0;
+            for (; b + 2 < nb; b += 2) {                  // two full batches per trip: no register copies between them
+                ep += ld;
+                const EB n1 = load_batch(ep);
+                hop_batch_n<T, R>(xs_bytes, pk, kGatherBatch, acc);
+                ep += ld;
+                pk = load_batch(ep);
+                hop_batch_n<T, R>(xs_bytes, n1, kGatherBatch, acc);
+            }
+            if (b + 1 < nb) {
                 ep += ld;
                 const EB nxt = load_batch(ep);
                 hop_batch_n<T, R>(xs_bytes, pk, kGatherBatch, acc);
