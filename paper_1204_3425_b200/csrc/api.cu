@@ -350,27 +350,44 @@ void gather_launch_shape(const hubbard_model *m, size_t smem, int *per_sm, int *
     *threads = std::max(32, kGatherMaxThreads / n / 32 * 32);
 }
 
-// Folded Lanczos form of variant GATHER: tensor-memory columns one CTA of the ROW sweep needs to park its tile of u_j
-// (one 16-byte piece per thread and gather iteration; a warp addresses a quarter of the 128 lanes), as the power of
-// two >= 32 that tcgen05.alloc takes.  0: the nine-pass form (knob 0; knob 1 = automatic and several CTAs per SM; or the
-// resident CTAs of an SM would need more than its 512 columns).  Knob 2 folds wherever the columns suffice.
+// Tensor-memory columns one CTA needs to keep one 16-byte item per thread and gather iteration of a sweep whose
+// contracted dimension is n_in (a warp addresses a quarter of the 128 lanes), as the power of two >= 32 that
+// tcgen05.alloc takes; 0 if the resident CTAs of an SM would need more than its 512 columns.
+int gather_tmem_cols(const hubbard_model *m, int64_t n_in, int words)
+{
+    const int R = gather_R(m);
+    const size_t es = m->dtype == HUBBARD_F32 ? 4 : 8;
+    const int64_t n_in_p = round_up(n_in, gather_align(m));
+    int per_sm, threads;
+    gather_launch_shape(m, gather_smem_bytes(n_in_p, R, es), &per_sm, &threads);
+    const int64_t n_it = (round_up(n_in_p, 32) + threads - 1) / threads;
+    const int64_t need = (int64_t)((threads / 32 + 3) / 4) * n_it * words;
+    int64_t cols = 32;
+    while (cols < need) cols *= 2;
+    return (cols * per_sm <= 512) ? (int)cols : 0;
+}
+
+// Folded Lanczos form of variant GATHER: columns the ROW sweep allocates to park its tile of u_j.  0: the nine-pass form
+// (knob 0; knob 1 = automatic and several CTAs per SM; or not enough tensor memory).  Knob 2 folds wherever it fits.
 int gather_fold_cols(const hubbard_model *m)
 {
     const int R = gather_R(m);
     if (!m->opt.gather_fold || R == 0) return 0;
     const size_t es = m->dtype == HUBBARD_F32 ? 4 : 8;
     if (R * es != 16) return 0;          // full-width tiles only (what AUTO runs as GATHER; narrower ones are test geometry)
-    const int64_t dd_p = round_up(m->dn.dim, gather_align(m));
-    int per_sm, threads;
-    gather_launch_shape(m, gather_smem_bytes(dd_p, R, es), &per_sm, &threads);
     // automatic: only where one tile fills the SM (C4).  Measured with the fold forced: C3 (2 CTAs per SM) no gain
     // (ROW + COL 0.376 ms either way), C2 (4 CTAs per SM, 4 tiles each) 10 % slower (the allocation is per launch).
+    int per_sm, threads;
+    gather_launch_shape(m, gather_smem_bytes(round_up(m->dn.dim, gather_align(m)), R, es), &per_sm, &threads);
     if (m->opt.gather_fold == 1 && per_sm != 1) return 0;
-    const int64_t n_it = (round_up(dd_p, 32) + threads - 1) / threads;
-    const int64_t need = (int64_t)((threads / 32 + 3) / 4) * n_it * (int64_t)(R * es / 4);
-    int64_t cols = 32;
-    while (cols < need) cols *= 2;
-    return (cols * per_sm <= 512) ? (int)cols : 0;
+    return gather_tmem_cols(m, m->dn.dim, 4);
+}
+
+// Folded form, COL sweep: columns for the first hop-entry batch (16 bytes) of every position of the up table
+int gather_ent_cols(const hubbard_model *m)
+{
+    if (gather_fold_cols(m) == 0 || !m->opt.gather_tmem_entries) return 0;
+    return gather_tmem_cols(m, m->up.dim, 4);
 }
 
 template <typename T, int R, typename E, bool COL, bool LZ, bool FOLD>
@@ -418,6 +435,7 @@ int launch_gather(hubbard_model *m, GatherArgs<T> A, cudaStream_t st)
         int rc = ensure_partials(m, (int64_t)m->sm_count * 8); if (rc) return rc;
         A.partials = m->d_partial;
         A.fold_cols = gather_fold_cols(m);
+        A.ent_cols = COL ? gather_ent_cols(m) : 0;
     }
     if (!A.in.e16) {
         if constexpr (sizeof(T) == 4) {
@@ -1447,6 +1465,7 @@ const OptKey kOptKeys[] = {
     {"gather_nosymmetry", &hub::DebugOptions::gather_nosymmetry, true, 0, 1},
     {"gather_ctas", &hub::DebugOptions::gather_ctas, false, 1, 4},
     {"gather_fold", &hub::DebugOptions::gather_fold, false, 0, 2},
+    {"gather_tmem_entries", &hub::DebugOptions::gather_tmem_entries, false, 0, 1},
     {"apply_pure_gather", &hub::DebugOptions::apply_pure_gather, false, 0, 1},
     {"twosweep_old_row", &hub::DebugOptions::twosweep_old_row, false, 0, 1},
     {"row_R", &hub::DebugOptions::row_R, false, 0, 4},

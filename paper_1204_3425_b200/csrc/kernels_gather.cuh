@@ -90,6 +90,9 @@ struct GatherArgs {
     // Lanczos, folded (eight-pass) form: tensor-memory columns the ROW sweep allocates to park u_j (0: nine-pass form,
     // the COL sweep reads u_j in CT)
     int fold_cols;
+    // Folded form, COL sweep: tensor-memory columns to keep the FIRST batch of hop entries of every position this CTA's
+    // threads own (the same positions in every tile) for the whole launch; 0: all entry batches come from L2
+    int ent_cols;
 };
 
 template <typename T, int N>
@@ -597,6 +600,61 @@ gather_sweep_kernel(GatherArgs<T> A)
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         tcol = tmem_base_s + (((uint32_t)(wv & 3) * 32u) << 16) + (uint32_t)(wv >> 2) * (uint32_t)(n_it * WPP);
     }
+    // Folded COL sweep: the first batch of a position's hop entries is what a thread waits for longest (it is requested
+    // one short partial batch ahead; ncu: a third of the sweep's stall samples).  A thread gathers for the SAME positions
+    // in every tile, so their first batches (16 bytes each, packed 16-bit entries) are parked in tensor memory once per
+    // launch and come back with tcgen05.ld: no L2 round trip at the position switch, a third of the entry traffic gone.
+    constexpr bool tment_k = COL && fold && sizeof(E) == 2;     // (instantiations that contain the tensor-memory path)
+    const bool tment = tment_k && A.ent_cols > 0;
+    constexpr int WPE = 4;                                      // 32-bit columns per parked batch
+    if (tment_k) {
+        if (tment) {
+            if (wv == 0) tmem_alloc(&tmem_base_s, (uint32_t)A.ent_cols);
+            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+            __syncthreads();
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            tcol = tmem_base_s + (((uint32_t)(wv & 3) * 32u) << 16) + (uint32_t)(wv >> 2) * (uint32_t)(n_it * WPE);
+            for (int it = 0; it < n_it; ++it) {
+                const int i = pos_of(it);
+                if (i >= n_in_w) continue;
+                const EB e0 = load_batch(reinterpret_cast<const EB *>(ent) + i);
+                uint32_t ew[WPE];
+#pragma unroll
+                for (int k = 0; k < WPE; ++k) ew[k] = e0.v[k];
+                tmem_st<WPE>(tcol + (uint32_t)(it * WPE), ew);
+            }
+            tmem_wait_st();
+        } else if (wv == 0) {
+            // (a CTA of a kernel that contains tcgen05.alloc holds the SM's allocation permit until it gives it up)
+            asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+        }
+    }
+    // first batch of the entries of this thread's position in gather iteration it_ (requested; see first_batch_ready)
+    auto first_batch = [&](int it_) {
+        EB e;
+        if constexpr (tment_k) {
+            if (tment) {
+                uint32_t ew[WPE] = {0u, 0u, 0u, 0u};
+                if (it_ < n_it) tmem_ld<WPE>(tcol + (uint32_t)(it_ * WPE), ew);
+#pragma unroll
+                for (int k = 0; k < WPE; ++k) e.v[k] = ew[k];
+                return e;
+            }
+        }
+        return load_batch(reinterpret_cast<const EB *>(ent) + min(pos_of(it_), n_in_w - 1));
+    };
+    auto first_batch_ready = [&](EB &e) {
+        if constexpr (tment_k) {
+            if (tment) {
+                uint32_t ew[WPE];
+#pragma unroll
+                for (int k = 0; k < WPE; ++k) ew[k] = e.v[k];
+                tmem_wait_ld<WPE>(ew);
+#pragma unroll
+                for (int k = 0; k < WPE; ++k) e.v[k] = ew[k];
+            }
+        }
+    };
     // piece of position i of the current tile
     auto poff = [&](int i) { return S == 1 ? (int64_t)i : (int64_t)(i / R) * (S * R) + i % R; };
 
@@ -703,10 +761,11 @@ gather_sweep_kernel(GatherArgs<T> A)
             for (int r = 0; r < R; ++r) so[r] = (o0 + r < du) ? A.st_out[o0 + r] : 0u;
         }
         // every position has >= 1 (padding) batch; the table has n_in_w batches per plane, a block may have more threads
-        EB pk = load_batch(reinterpret_cast<const EB *>(ent) + min(pos_of(0), n_in_w - 1));
+        EB pk = first_batch(0);
         for (int it = 0; it < n_it; ++it) {
             const int i = pos_of(it);
-            if (i >= n_in_w) continue;                    // whole warps: a partly filled last stripe
+            first_batch_ready(pk);                        // (before the skip: a tensor-memory load must not stay pending)
+            if (i >= n_in_w) continue;                    // whole warps: a partly filled last stripe (the last iteration only)
             const bool valid = i < n_in;
             const bool inpad = i < n_in_p;
             const int n = (int)wsl_s[i >> 5];                // warp-uniform, >= 1
@@ -767,7 +826,7 @@ gather_sweep_kernel(GatherArgs<T> A)
                 pk = nxt;
             }
             {
-                const EB nxt = load_batch(reinterpret_cast<const EB *>(ent) + min(pos_of(it + 1), n_in_w - 1));
+                const EB nxt = first_batch(it + 1);
                 hop_batch_n<T, R>(xs_bytes, pk, n - (nb - 1) * kGatherBatch, acc);    // 1..8 entries, warp-uniform
                 pk = nxt;
             }
@@ -840,10 +899,10 @@ gather_sweep_kernel(GatherArgs<T> A)
         }
     }
 
-    if (park) {
+    if (park || tment) {
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
         __syncthreads();
-        if (wv == 0) tmem_dealloc(tmem_base_s, (uint32_t)A.fold_cols);
+        if (wv == 0) tmem_dealloc(tmem_base_s, (uint32_t)(park ? A.fold_cols : A.ent_cols));
     }
     if (LZ) {
         const double sblk = block_sum(racc, red);

@@ -81,6 +81,7 @@ struct DebugOptions {
     int gather_nosort = 0;          // 1: the Lanczos work vectors keep the basis order (no internal reordering)
     int gather_nosymmetry = 0;      // 1: internal order from hop counts only (no lattice-symmetry orbits)
     int gather_ctas = 4;            // CTAs per SM for small tiles
+    int gather_tmem_entries = 1;    // folded form: the COL sweep keeps the first hop-entry batch of its positions in tensor memory
     int gather_fold = 1;            // eight-pass Lanczos form (- b f_{j-1} folded into the ROW sweep through tensor memory):
                                     // 0 never, 1 where one tile fills the SM (automatic), 2 wherever the tensor memory suffices
     int apply_pure_gather = 0;      // 1: plain hubbard_apply as two gather sweeps instead of the hybrid
