@@ -242,6 +242,34 @@ __device__ __forceinline__ P ld_once(const P *p)
         return *reinterpret_cast<const P *>(&u);
     }
 }
+#ifndef GS_EARLY_FIRST
+#define GS_EARLY_FIRST 1
+#endif
+// staging loads of the folded ROW sweep
+#ifndef GS_PARK_UNROLL
+#define GS_PARK_UNROLL 1
+#endif
+#ifndef GS_PARK_NA
+#define GS_PARK_NA 0
+#endif
+template <typename P>
+__device__ __forceinline__ P ld_stage(const P *p)
+{
+#if GS_PARK_NA
+    if constexpr (sizeof(P) == 16) {
+        uint32_t a, b, c, d;
+        asm volatile("ld.global.L1::no_allocate.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(a), "=r"(b), "=r"(c), "=r"(d) : "l"(p));
+        const uint32_t u[4] = {a, b, c, d};
+        P o;
+        memcpy(&o, u, 16);
+        return o;
+    } else {
+        return ld_once<1>(p);
+    }
+#else
+    return ld_once<1>(p);
+#endif
+}
 template <int BIT, typename P>
 __device__ __forceinline__ void st_once(P *p, const P &v)
 {
@@ -671,25 +699,33 @@ gather_sweep_kernel(GatherArgs<T> A)
                 // own in the epilogue (whole warps: the tensor-memory accesses are warp-collective)
                 const PR *fsrc = reinterpret_cast<const PR *>(A.Frt) + tbase;
                 PR *wdst = reinterpret_cast<PR *>(A.Qrt) + tbase;
-                for (int it = 0; it < n_it; ++it) {
-                    const int i = pos_of(it);
-                    if (i >= n_in_w) continue;
-                    PR v, f;
+                for (int it0 = 0; it0 < n_it; it0 += GS_PARK_UNROLL) {
+                    PR v[GS_PARK_UNROLL], f[GS_PARK_UNROLL];
 #pragma unroll
-                    for (int r = 0; r < R; ++r) v.v[r] = f.v[r] = T(0);
-                    if (i < n_in_p) { v = ld_once<1>(src + poff(i)); f = ld_once<1>(fsrc + poff(i)); }
+                    for (int u = 0; u < GS_PARK_UNROLL; ++u) {
+                        const int i = pos_of(it0 + u);
 #pragma unroll
-                    for (int r = 0; r < R; ++r) {
-                        v.v[r] = v.v[r] - ac * f.v[r];
-                        racc += (double)v.v[r] * (double)v.v[r];
+                        for (int r = 0; r < R; ++r) v[u].v[r] = f[u].v[r] = T(0);
+                        if (it0 + u < n_it && i < n_in_p) { v[u] = ld_stage(src + poff(i)); f[u] = ld_stage(fsrc + poff(i)); }
                     }
-                    if (i < n_in_p) {
-                        st_once<1>(wdst + poff(i), v);
-                        Xs[i] = v;
+#pragma unroll
+                    for (int u = 0; u < GS_PARK_UNROLL; ++u) {
+                        const int it = it0 + u;
+                        const int i = pos_of(it);
+                        if (it >= n_it || i >= n_in_w) continue;
+#pragma unroll
+                        for (int r = 0; r < R; ++r) {
+                            v[u].v[r] = v[u].v[r] - ac * f[u].v[r];
+                            racc += (double)v[u].v[r] * (double)v[u].v[r];
+                        }
+                        if (i < n_in_p) {
+                            st_once<1>(wdst + poff(i), v[u]);
+                            Xs[i] = v[u];
+                        }
+                        uint32_t fw[WPP];
+                        memcpy(fw, &f[u], sizeof(PR));
+                        tmem_st<WPP>(tcol + (uint32_t)(it * WPP), fw);
                     }
-                    uint32_t fw[WPP];
-                    memcpy(fw, &f, sizeof(PR));
-                    tmem_st<WPP>(tcol + (uint32_t)(it * WPP), fw);
                 }
                 tmem_wait_st();
             } else if (!COL) {
@@ -810,7 +846,15 @@ gather_sweep_kernel(GatherArgs<T> A)
             // batch of this thread's next state
             const EB *ep = reinterpret_cast<const EB *>(ent) + i;
             const int nb = (n + kGatherBatch - 1) / kGatherBatch;
+            // the first batch of the NEXT position: the fp32 ROW sweep requests it a whole position ahead, the others just
+            // before this position's last batch (the folded COL sweep from tensor memory)
+            EB nxtpos;
+            // (measured on C4: ROW fp32 0.989 -> 0.966 ms, fp64 1.806 -> 1.826 ms; the COL sweeps have no registers for it)
+            constexpr bool early_first = GS_EARLY_FIRST && !COL && sizeof(T) == 4;
+            if (early_first) nxtpos = first_batch(it + 1);
             int b = 0;
+            // (the nine-pass COL sweep, which holds two epilogue operands over the gather, spills 8 bytes for this and is still
+            // faster with it: C3 0.173 against 0.188 ms)
             for (; b + 2 < nb; b += 2) {                  // two full batches per trip: no register copies between them
                 ep += ld;
                 const EB n1 = load_batch(ep);
@@ -819,16 +863,16 @@ gather_sweep_kernel(GatherArgs<T> A)
                 pk = load_batch(ep);
                 hop_batch_n<T, R>(xs_bytes, n1, kGatherBatch, acc);
             }
-            if (b + 1 < nb) {
+            for (; b + 1 < nb; ++b) {
                 ep += ld;
                 const EB nxt = load_batch(ep);
                 hop_batch_n<T, R>(xs_bytes, pk, kGatherBatch, acc);
                 pk = nxt;
             }
             {
-                const EB nxt = first_batch(it + 1);
+                if (!early_first) nxtpos = first_batch(it + 1);
                 hop_batch_n<T, R>(xs_bytes, pk, n - (nb - 1) * kGatherBatch, acc);    // 1..8 entries, warp-uniform
-                pk = nxt;
+                pk = nxtpos;
             }
             PR xi;
 #pragma unroll
