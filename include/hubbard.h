@@ -323,6 +323,8 @@ int64_t hubbard_launch_count(const hubbard_model *m);
  *                             where one tile fills an SM's shared memory (C4), 2 wherever the SM's 512 tensor-memory
  *                             columns suffice for its resident CTAs, 0 never = the nine-pass form (the COL sweep reads
  *                             u_j).  DESIGN.md 2 (readings) and 4.2
+ *   "gather_tmem_entries" (0/1)  folded form: the COL sweep keeps the first hop-entry batch of each of its positions in
+ *                             tensor memory for the whole launch (default 1; 0 = every batch is loaded from L2)
  *   "apply_pure_gather" (0/1) plain hubbard_apply as two gather sweeps instead of the hybrid
  *   "twosweep_old_row" (0/1)  AUTO's TWOSWEEP fallback keeps the first row kernel
  *   "row_R" (0-4), "strip_mb" (1-1024), "strip_rb"   geometry of variant TWOSWEEP (0 = automatic)
