@@ -438,6 +438,11 @@ def test_gather_lanczos_folded_and_nine_pass_forms(name, ns, nu, nd, bonds, ctas
         a2, b2 = m.lanczos_run(x, 40)
         assert np.array_equal(alpha, a2) and np.array_equal(beta, b2)      # deterministic, and tensor memory is released
         got[fold] = (alpha, beta)
+        if fold and m.hubbard_debug_get("resolved_gather_fold"):
+            # the folded COL sweep with its first entry batches from L2 instead of tensor memory: the same arithmetic
+            m.hubbard_debug_set("gather_tmem_entries", 0)
+            a3, b3 = m.lanczos_run(x, 40)
+            assert np.array_equal(alpha, a3) and np.array_equal(beta, b3)
     # the two forms differ only in rounding (the coefficient of f_j is |q|^2 - a^2 instead of |w|^2)
     assert np.max(np.abs(got[0][0][:30] - got[2][0][:30])) <= tol_c * 20
 
